@@ -1,0 +1,142 @@
+"""Pins for the oracle's whole tracer and estimator."""
+import math
+
+import numpy as np
+
+from paper_2604_07617_b200 import workloads as W
+
+
+def _rk4_bruteforce(O, f, p, x0, T, nsteps):
+    """Classical fixed-step RK4 on the oracle's RHS: shares only the RHS with the DP5 tracer."""
+    y = np.zeros(4)
+    y[0], y[1], y[2], y[3] = x0[0] * math.cos(x0[1]), x0[0] * math.sin(x0[1]), x0[2], x0[3]
+    mu = O.mu_init(f, p, x0)
+    h = T / nsteps
+    t = 0.0
+    for _ in range(nsteps):
+        k1, _ = O.rhs(f, p, mu, t, y)
+        k2, _ = O.rhs(f, p, mu, t + h / 2, y + h / 2 * k1)
+        k3, _ = O.rhs(f, p, mu, t + h / 2, y + h / 2 * k2)
+        k4, _ = O.rhs(f, p, mu, t + h, y + h * k3)
+        y = y + h / 6 * (k1 + 2 * k2 + 2 * k3 + k4)
+        t += h
+    return np.array([math.hypot(y[0], y[1]), math.atan2(y[1], y[0]), y[2], y[3]])
+
+
+def test_trace_agrees_with_fine_step_rk4(oracle):
+    """Brute force: the adaptive DP5 trace converges to a fixed-step RK4 solution of the same RHS.
+    Global error of an accepted-step sequence is bounded by ~ n_steps * rtol * scale (Eq. 4)."""
+    O = oracle
+    cfg = W.config(0, n=4, T=1e-5)
+    f = O.Field(cfg["field"])
+    p9 = O.make_params(cfg["params"])
+    r9 = O.trace(f, p9, cfg["x0"])
+    assert np.all(r9["status"] == 0) and np.all(r9["tstop"] == 1e-5)
+    r12 = O.trace(f, O.make_params(dict(cfg["params"], rtol=1e-12, atol=1e-15)), cfg["x0"])
+    nst = int(r9["nacc"].max()) * 12
+    scale = np.array([1.0, 1.0, 10.0, W.V_TOTAL])
+    for i in range(4):
+        ref = _rk4_bruteforce(O, f, p9, cfg["x0"][:, i], 1e-5, nst)
+        for r, tol in ((r12, 1e-8), (r9, 3 * r9["nacc"][i] * 1e-9)):
+            d = r["xf"][:, i] - ref
+            d[1] = math.remainder(d[1], 2 * math.pi)
+            assert np.all(np.abs(d) < tol * scale), (i, d, tol)
+
+
+def test_tolerance_refinement_converges(oracle):
+    """The end state moves toward a tight-tolerance reference as rtol shrinks."""
+    O = oracle
+    cfg = W.config(0, n=3, T=1e-5)
+    f = O.Field(cfg["field"])
+    ends = {}
+    for rtol in (1e-6, 1e-8, 1e-11):
+        pd = dict(cfg["params"], rtol=rtol, atol=rtol * 1e-3)
+        ends[rtol] = O.trace(f, O.make_params(pd), cfg["x0"])["xf"]
+    e6 = np.abs(ends[1e-6][0] - ends[1e-11][0]).max()
+    e8 = np.abs(ends[1e-8][0] - ends[1e-11][0]).max()
+    # bounded by n_steps * rtol (Eq. 4 is a per-step control), and monotone in the tolerance
+    assert e8 < e6 and e8 < 200 * 1e-8 and e6 < 200 * 1e-6
+
+
+def test_stop_logic(oracle):
+    O = oracle
+    cfg = W.config(0, n=8, T=2e-6)
+    f = O.Field(cfg["field"])
+    x0 = cfg["x0"].copy()
+    x0[0, 0] = 1.2                                  # born outside: status 1, t_stop 0, state returned
+    x0[0, 1] = 0.999
+    x0[3, 1] = 0.05 * W.V_TOTAL                     # barely trapped near the edge, drifts out or stays
+    r = O.trace(f, O.make_params(cfg["params"]), x0)
+    assert r["status"][0] == 1 and r["tstop"][0] == 0.0 and np.array_equal(r["xf"][:, 0], x0[:, 0])
+    assert r["nacc"][0] == 0
+    alive = r["status"] == 0
+    assert np.all(r["tstop"][alive] == 2e-6)        # the last step lands exactly on T (reading S4)
+    lost = r["status"] == 1
+    assert np.all(r["xf"][0][lost] >= 1.0)          # loss = first accepted state with s >= 1 (S5)
+    assert np.all(r["xf"][0][alive] < 1.0)
+    # max_steps => status 3 ; tiny max_consecutive_rejects with absurd dt0 => status 2
+    pd = dict(cfg["params"], max_steps=5)
+    r3 = O.trace(f, O.make_params(pd), cfg["x0"])
+    assert np.all(r3["status"] == 3) and np.all(r3["nacc"] + r3["nrej"] == 5)
+    pd = dict(cfg["params"], dt0=1e-3, dtmax=1e-3, max_consecutive_rejects=2)
+    r2 = O.trace(f, O.make_params(pd), cfg["x0"])
+    assert np.all(r2["status"] == 2) and np.all(r2["nrej"] == 2)
+
+
+def test_particle_crossing_the_edge_is_lost_and_extrapolates(oracle):
+    """stages beyond s = 1 use the last cell's polynomial; tracing stops at s >= 1."""
+    O = oracle
+    cfg = W.config(0, n=64, T=1e-4)
+    f, p = O.Field(cfg["field"]), O.make_params(cfg["params"])
+    r = O.trace(f, p, cfg["x0"])
+    lost = np.flatnonzero(r["status"] == 1)
+    assert len(lost) >= 1
+    assert np.all(r["xf"][0][lost] >= 1.0) and np.all(r["xf"][0][lost] < 1.05)
+    assert np.all(r["tstop"][lost] < 1e-4) and np.all(r["tstop"][lost] > 0)
+    # table energy drift is interpolation-limited (reading Q3): same order as O(h^4)
+    keep = np.flatnonzero(r["status"] == 0)
+    B0v = O.tricubic_many(f, cfg["x0"][:3])[0]
+    Bf = O.tricubic_many(f, r["xf"][:3])[0]
+    mu = (W.V_TOTAL ** 2 - cfg["x0"][3] ** 2) / (2 * B0v)
+    E = 0.5 * r["xf"][3] ** 2 + mu * Bf
+    drift = np.abs(E / (0.5 * W.V_TOTAL ** 2) - 1)
+    assert np.median(drift[keep]) < 5e-6
+
+
+def test_cartesian_trace_on_tables_conserves_pphi(oracle):
+    """Config 3 at reduced size: canonical toroidal momentum and energy from tabulated columns."""
+    O = oracle
+    cfg = W.config(3, n=6, T=2e-5, ncell=[24, 24, 4])
+    f, p = O.Field(cfg["field"]), O.make_params(cfg["params"])
+    r = O.trace(f, p, cfg["x0"])
+    assert np.all(r["status"] == 0)
+
+    def inv(x):
+        R = np.hypot(x[0], x[1])
+        v = O.tricubic_many(f, np.array([R, x[2], np.arctan2(x[1], x[0])]))
+        modB = np.sqrt(v[0] ** 2 + v[1] ** 2 + v[2] ** 2)
+        return R, v, modB
+
+    R0_, v0, B0_ = inv(cfg["x0"])
+    R1_, v1, B1_ = inv(r["xf"])
+    mu = (W.V_TOTAL ** 2 - cfg["x0"][3] ** 2) / (2 * B0_)
+    E1 = 0.5 * r["xf"][3] ** 2 + mu * B1_
+    assert np.max(np.abs(E1 / (0.5 * W.V_TOTAL ** 2) - 1)) < 1e-6
+    P0 = W.ALPHA_MASS * R0_ * v0[1] / B0_ * cfg["x0"][3] + W.ALPHA_CHARGE * v0[6]
+    P1 = W.ALPHA_MASS * R1_ * v1[1] / B1_ * r["xf"][3] + W.ALPHA_CHARGE * v1[6]
+    assert np.max(np.abs(P1 - P0)) < 1e-6 * W.ALPHA_CHARGE * W.PSI_EDGE_CYL
+
+
+def test_estimator_matches_numpy(oracle):
+    O = oracle
+    rng = np.random.default_rng(43)
+    status = rng.integers(0, 3, size=1000).astype(np.int32)
+    tstop = rng.random(1000)
+    out = O.estimate(0, status=status, tstop=tstop)
+    g = (status == 1).astype(float)
+    assert out[2] == g.sum() and abs(out[0] - g.mean()) < 1e-15
+    assert abs(out[1] - math.sqrt(g.mean() * (1 - g.mean()) / (len(g) - 1))) < 1e-12
+    out = O.estimate(1, status=status, tstop=tstop)
+    assert abs(out[0] - tstop.mean()) < 1e-14 and abs(out[1] - tstop.std(ddof=0) / math.sqrt(999)) < 1e-12
+    out = O.estimate(2, status=status, tstop=tstop, g_user=tstop ** 2)
+    assert abs(out[0] - (tstop ** 2).mean()) < 1e-14

@@ -1,0 +1,184 @@
+/*
+ * catapult.h -- C-ABI of the B200-native CATAPULT hot path (arxiv/paper_2604_07617).
+ *
+ * What it computes (PAPER.md = the paper's text; DESIGN.md lists every reading of a silent point):
+ *   per-particle tracing of the Littlejohn guiding-centre equations (Eq. 3) in
+ *   Boozer (s,theta,zeta,vpar) and Cartesian (x,y,z,vpar) form with Dormand-Prince 5(4) adaptive
+ *   steps (Eq. 4 at PAPER.md:85), every stage evaluating a local tricubic interpolant
+ *   of gridded field quantities, stopping at the loss boundary or at T
+ *   (PAPER.md:57-59), and the Monte-Carlo estimate of Eq. 2.
+ *
+ * Conventions
+ *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers; all are owned by the caller,
+ *     the library never frees them.  `stream` is a cudaStream_t passed as void* (NULL = default
+ *     stream).  All work runs on the device that is current when the call is made.
+ *   - Every call returns a catapult_status; no exception crosses the boundary;
+ *     catapult_last_error() returns a thread-local message for the last failing call.
+ *   - Calls validate their arguments synchronously, enqueue work on `stream` and do not
+ *     synchronise, except the *_host variants and catapult_estimate with a non-NULL h_out, which
+ *     return after their results are in host memory.
+ *   - There is no CPU fallback anywhere: without a CUDA device every compute call fails with
+ *     CATAPULT_ECUDA.
+ *   - Particle arrays are structure-of-arrays: x[4][n] means component c of particle i at
+ *     x[c*n + i].  Boozer state = (s, theta, zeta, vpar); Cartesian state = (x, y, z, vpar).
+ */
+#ifndef CATAPULT_H
+#define CATAPULT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  CATAPULT_OK = 0,
+  CATAPULT_EINVAL = 1,       /* bad argument (NULL required pointer, n<0, ncell<1, non-finite T/rtol/atol ...) */
+  CATAPULT_ENOMEM = 2,       /* device or host allocation failed */
+  CATAPULT_ECUDA = 3,        /* CUDA runtime error (message in catapult_last_error) */
+  CATAPULT_EUNSUPPORTED = 4  /* valid but not built (e.g. non-vacuum Boozer I != 0) */
+} catapult_status;
+
+#define CATAPULT_COORD_BOOZER 0 /* grid (s,theta,zeta); particles (s,theta,zeta,vpar)            */
+#define CATAPULT_COORD_CYL 1    /* grid (R,Z,phi); particles (x,y,z,vpar)       */
+
+/* Column (quantity) order of the gridded data.
+   Boozer vacuum: |B|, d|B|/ds, d|B|/dtheta, d|B|/dzeta            -> nquant = 4
+   Cylindrical grid (R3): B_R, B_phi, B_Z, d|B|/dR, (1/R) d|B|/dphi, d|B|/dZ,
+                                    psi (loss level function)        -> nquant = 7 */
+#define CATAPULT_NQUANT_BOOZER 4
+#define CATAPULT_NQUANT_CYL 7
+
+/* particle status */
+#define CATAPULT_ST_REACHED_T 0
+#define CATAPULT_ST_LOST 1      /* s >= 1 (Boozer) or psi >= psi_edge (Cartesian) */
+#define CATAPULT_ST_STALLED 2   /* max_consecutive_rejects rejected attempts in a row */
+#define CATAPULT_ST_MAXSTEPS 3  /* max_steps attempts used */
+
+typedef struct {
+  int32_t coord;    /* CATAPULT_COORD_* */
+  int32_t ncell[3]; /* interpolant cells per dimension, slowest -> fastest;
+                       unique nodes per dimension = 3*ncell+1 */
+  int32_t nfp;      /* field periods: the last grid dimension spans [lo, lo + 2pi/nfp) */
+  int32_t nquant;   /* m, must equal CATAPULT_NQUANT_* of `coord` */
+  double lo[3], hi[3]; /* Boozer: [0,1],[0,2pi],[0,2pi/nfp]; cyl: [Rmin,Rmax],[Zmin,Zmax],[0,2pi/nfp].
+                          theta, zeta and phi are periodic with period hi-lo; s, R, Z extrapolate
+                          with the nearest cell's cubic outside [lo,hi] */
+  double G0, I0;       /* Boozer covariant components, constants (vacuum: I0 must be 0) */
+  double iota0, iota1; /* rotational transform iota(s) = iota0 + iota1*s */
+  double psi0;         /* Boozer: toroidal flux/(2pi) at s=1; cyl: psi_edge (loss level) */
+} catapult_field_desc;
+
+typedef struct catapult_field catapult_field; /* opaque; owns the per-cell coefficient tables */
+
+typedef struct {
+  double mass, charge, energy; /* shared by all particles; v_total = sqrt(2E/m) */
+  double T;                    /* end time of the trace (absolute time), > 0 and finite        */
+  double rtol, atol;           /* Eq. 4; atol is multiplied by v_total for vpar
+                                                                                   */
+  double dt0, dtmax;           /* initial / maximum step; <= 0 selects the defaults of DESIGN.md S3 */
+  int64_t max_steps;           /* attempts per particle per call; 0 = unlimited                 */
+  int32_t max_consecutive_rejects; /* 0 = 500                                                   */
+  int32_t saw_on;              /* 1: shear Alfven wave, Boozer only              */
+  int32_t saw_m, saw_n;        /* Phi = Phi0 exp(-(s-s0)^2/w2) sin(m theta - n zeta + omega t)  */
+  double saw_Phi0, saw_s0, saw_w2, saw_omega;
+} catapult_trace_params;
+
+/* ---- field tables ------------------------------------------------
+ * catapult_field_build: d_nodes holds the unique nodes [nquant][3*ncell0+1][3*ncell1+1][3*ncell2+1]
+ * (last index fastest).  A device kernel gathers, for every cell, the 4x4x4 nodal block of every
+ * quantity (shared faces duplicated) into the cell-major table
+ * [cell][quantity][64] (cell = (i0*ncell1+i1)*ncell2+i2, node = (a*4+b)*4+c): one cell's
+ * coefficients of one quantity are four 128-byte lines.  *out owns the table; d_nodes may be
+ * freed once the stream has run.  Errors: EINVAL (NULL, ncell<1, nquant mismatch, hi<=lo),
+ * EUNSUPPORTED (Boozer I0 != 0), ENOMEM, ECUDA. */
+catapult_status catapult_field_build(const catapult_field_desc *desc, const double *d_nodes,
+                                     void *stream, catapult_field **out);
+/* same with HOST nodes: copies them to the device, builds, synchronises, frees the staging copy */
+catapult_status catapult_field_build_host(const catapult_field_desc *desc, const double *h_nodes,
+                                          catapult_field **out);
+catapult_status catapult_field_destroy(catapult_field *f);
+/* bytes of the device coefficient table (64 * ncells * nquant * 8) */
+size_t catapult_field_table_bytes(const catapult_field *f);
+
+/* test hook: tricubic values of all quantities at npts points given in GRID coordinates
+   d_pts[3][npts] ((s,theta,zeta) or (R,Z,phi), unreduced) -> d_out[nquant][npts] */
+catapult_status catapult_field_eval(const catapult_field *f, int64_t npts, const double *d_pts,
+                                    double *d_out, void *stream);
+/* test hook: writes the table in the paper's own layout: row = cell*64 + node,
+   column = quantity, d_out[(cell*64+node)*nquant + q]; 64*ncells*nquant doubles */
+catapult_status catapult_field_export_rows(const catapult_field *f, double *d_out, void *stream);
+
+/* ---- tracing --------------------------------------------------------------
+ * catapult_trace: each of the n particles starts at t=0 from d_x0[4][n] and is advanced with
+ * DP5 steps until min(tau, T): d_xf[4][n] = last observed state in the input's
+ * coordinates (Boozer theta in (-pi,pi], zeta unreduced), d_tstop[n] = min(tau,T),
+ * d_status[n] = CATAPULT_ST_*; d_nacc/d_nrej[n] (may be NULL) = accepted / rejected attempts.
+ * A particle already outside at t=0 is returned unchanged with status LOST and t_stop = 0.
+ * d_counters (may be NULL): 8 uint64 accumulated (atomically added) by the kernel:
+ *   [0] accepted steps, [1] rejected attempts, [2] particles finished at T, [3] lost,
+ *   [4] stalled, [5] max_steps, [6] right-hand-side evaluations, [7] cell-table (re)loads. */
+catapult_status catapult_trace(const catapult_field *f, const catapult_trace_params *p, int64_t n,
+                               const double *d_x0, double *d_xf, double *d_tstop,
+                               int32_t *d_status, uint32_t *d_nacc, uint32_t *d_nrej,
+                               uint64_t *d_counters, void *stream);
+/* Restartable form: all arrays are in/out.  Particles whose d_status is REACHED_T are advanced
+ * from their own time d_t[i] to p->T with controller step d_dt[i] and magnetic moment d_mu[i]
+ * (per unit mass); others are left untouched.  d_nacc/d_nrej (may be NULL) are incremented.
+ * catapult_trace_init fills (t=0, dt=dt0, mu from the tabulated |B|, status REACHED_T or LOST)
+ * so that init + continue(T) equals catapult_trace(T) exactly. */
+catapult_status catapult_trace_init(const catapult_field *f, const catapult_trace_params *p,
+                                    int64_t n, const double *d_x, double *d_t, double *d_dt,
+                                    double *d_mu, int32_t *d_status, void *stream);
+catapult_status catapult_trace_continue(const catapult_field *f, const catapult_trace_params *p,
+                                        int64_t n, double *d_x, double *d_t, double *d_dt,
+                                        double *d_mu, int32_t *d_status, uint32_t *d_nacc,
+                                        uint32_t *d_nrej, uint64_t *d_counters, void *stream);
+/* HOST-buffer form of catapult_trace: copies h_x0 to the device, traces, copies the results back
+   and synchronises.  h_nacc/h_nrej/h_counters may be NULL. */
+catapult_status catapult_trace_host(const catapult_field *f, const catapult_trace_params *p,
+                                    int64_t n, const double *h_x0, double *h_xf, double *h_tstop,
+                                    int32_t *h_status, uint32_t *h_nacc, uint32_t *h_nrej,
+                                    uint64_t *h_counters);
+/* HOST-buffer form of catapult_trace_continue: the state arrays (all required except h_nacc,
+   h_nrej, h_counters) are copied to the device, advanced to p->T, copied back; synchronises. */
+catapult_status catapult_trace_continue_host(const catapult_field *f, const catapult_trace_params *p,
+                                             int64_t n, double *h_x, double *h_t, double *h_dt,
+                                             double *h_mu, int32_t *h_status, uint32_t *h_nacc,
+                                             uint32_t *h_nrej, uint64_t *h_counters);
+/* test hook: ONE attempted DP5 step of size d_h[i] from state d_x[4][n] at time d_t[n] (mu taken
+   from the state as in catapult_trace_init): d_xnew[4][n], d_errratio[n] (Eq. 4),
+   d_k[7][4][n] = the seven stage derivatives in the stepped variables */
+catapult_status catapult_step_once(const catapult_field *f, const catapult_trace_params *p,
+                                   int64_t n, const double *d_x, const double *d_t,
+                                   const double *d_h, double *d_xnew, double *d_errratio,
+                                   double *d_k, void *stream);
+
+/* ---- estimate (Eq. 2) ----------------------------------------------------------
+ * g_kind 0: g = 1[status == LOST] (integer count, exact); 1: g = t_stop; 2: g = d_g_user.
+ * d_out[3] (device, required) = { mean, standard error sqrt((sum g^2/n - mean^2)/(n-1)), sum g }.
+ * Deterministic fixed-order tree.  If h_out != NULL the three doubles are also copied to the host
+ * and the stream is synchronised. */
+catapult_status catapult_estimate(int32_t g_kind, int64_t n, const int32_t *d_status,
+                                  const double *d_tstop, const double *d_g_user, double *d_out,
+                                  double *h_out, void *stream);
+
+/* ---- measurement hooks (roofline denominators) ---------------------
+ * catapult_measure_fp64_peak: runs a register-only DFMA kernel on every SM and returns the
+ * sustained double-precision rate in FLOP/s (2 per DFMA).
+ * catapult_measure_l2_bandwidth: repeatedly reads a `bytes`-sized device buffer (choose it below
+ * the L2 size) with 16-byte loads and returns bytes/s.  Both synchronise. */
+catapult_status catapult_measure_fp64_peak(double *flops_per_s);
+catapult_status catapult_measure_l2_bandwidth(size_t bytes, double *bytes_per_s);
+/* launch geometry the tracer uses on the current device: persistent blocks and threads per block */
+catapult_status catapult_trace_launch_shape(const catapult_field *f, const catapult_trace_params *p,
+                                            int32_t *blocks, int32_t *threads);
+
+const char *catapult_last_error(void);
+const char *catapult_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CATAPULT_H */

@@ -1,0 +1,465 @@
+// C-ABI entry points of libcatapult.so (include/catapult.h): argument validation, table ownership,
+// parameter packing and stream-ordered launches.  No arithmetic of the method lives here.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "gc_device.cuh"
+
+namespace catapult {
+
+static thread_local std::string g_last_error;
+
+void set_error(const std::string& msg) { g_last_error = msg; }
+
+catapult_status cuda_fail(cudaError_t e, const char* what) {
+  char buf[512];
+  std::snprintf(buf, sizeof(buf), "CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), what);
+  set_error(buf);
+  return e == cudaErrorMemoryAllocation ? CATAPULT_ENOMEM : CATAPULT_ECUDA;
+}
+
+static catapult_status fail(catapult_status st, const char* msg) {
+  set_error(msg);
+  return st;
+}
+
+static const double E_CHARGE = 1.602176634e-19;
+static const double PI = 3.14159265358979323846;
+
+static catapult_status validate_desc(const catapult_field_desc* d) {
+  if (!d) return fail(CATAPULT_EINVAL, "desc is NULL");
+  if (d->coord != CATAPULT_COORD_BOOZER && d->coord != CATAPULT_COORD_CYL)
+    return fail(CATAPULT_EINVAL, "desc.coord must be CATAPULT_COORD_BOOZER or CATAPULT_COORD_CYL");
+  for (int i = 0; i < 3; ++i) {
+    if (d->ncell[i] < 1) return fail(CATAPULT_EINVAL, "desc.ncell must be >= 1");
+    if (!(std::isfinite(d->lo[i]) && std::isfinite(d->hi[i]) && d->hi[i] > d->lo[i]))
+      return fail(CATAPULT_EINVAL, "desc.lo/hi must be finite with hi > lo");
+  }
+  const int want = d->coord == CATAPULT_COORD_BOOZER ? CATAPULT_NQUANT_BOOZER : CATAPULT_NQUANT_CYL;
+  if (d->nquant != want) return fail(CATAPULT_EINVAL, "desc.nquant does not match desc.coord (4 Boozer, 7 cyl)");
+  if (d->nfp < 1) return fail(CATAPULT_EINVAL, "desc.nfp must be >= 1");
+  if (d->coord == CATAPULT_COORD_BOOZER) {
+    if (d->I0 != 0.0) return fail(CATAPULT_EUNSUPPORTED, "non-vacuum Boozer (I0 != 0) is not built");
+    if (!(std::isfinite(d->G0) && d->G0 != 0.0)) return fail(CATAPULT_EINVAL, "desc.G0 must be finite, non-zero");
+    if (!(std::isfinite(d->psi0) && d->psi0 != 0.0)) return fail(CATAPULT_EINVAL, "desc.psi0 must be finite, non-zero");
+  } else if (!std::isfinite(d->psi0)) {
+    return fail(CATAPULT_EINVAL, "desc.psi0 (psi_edge) must be finite");
+  }
+  return CATAPULT_OK;
+}
+
+static void fill_field_const(const catapult_field_desc& d, const double* table, FieldConst* fc) {
+  fc->table = table;
+  fc->coord = d.coord;
+  fc->m = d.nquant;
+  for (int i = 0; i < 3; ++i) {
+    fc->k[i] = d.ncell[i];
+    fc->lo[i] = d.lo[i];
+    fc->span[i] = d.hi[i] - d.lo[i];
+    fc->invspan[i] = 1.0 / fc->span[i];
+    const double h = fc->span[i] / (double)d.ncell[i];
+    fc->invh[i] = 1.0 / h;
+  }
+  fc->G = d.G0;
+  fc->invG = d.G0 != 0.0 ? 1.0 / d.G0 : 0.0;
+  fc->psi0 = d.psi0;
+  fc->invpsi0 = d.psi0 != 0.0 ? 1.0 / d.psi0 : 0.0;
+  fc->iota0 = d.iota0;
+  fc->iota1 = d.iota1;
+}
+
+static catapult_status make_trace_const(const catapult_field* f, const catapult_trace_params* p, TraceConst* tc,
+                                        int* model) {
+  if (!f) return fail(CATAPULT_EINVAL, "field is NULL");
+  if (!p) return fail(CATAPULT_EINVAL, "params is NULL");
+  if (!(std::isfinite(p->mass) && p->mass > 0.0 && std::isfinite(p->charge) && p->charge != 0.0 &&
+        std::isfinite(p->energy) && p->energy > 0.0))
+    return fail(CATAPULT_EINVAL, "mass, |charge| and energy must be finite and positive");
+  if (!(std::isfinite(p->T) && p->T > 0.0)) return fail(CATAPULT_EINVAL, "T must be finite and > 0");
+  if (!(std::isfinite(p->rtol) && p->rtol >= 0.0 && std::isfinite(p->atol) && p->atol >= 0.0 &&
+        (p->rtol > 0.0 || p->atol > 0.0)))
+    return fail(CATAPULT_EINVAL, "rtol/atol must be finite, non-negative, not both zero");
+  if (p->max_steps < 0 || p->max_consecutive_rejects < 0)
+    return fail(CATAPULT_EINVAL, "max_steps / max_consecutive_rejects must be >= 0");
+  if (p->saw_on) {
+    if (f->desc.coord != CATAPULT_COORD_BOOZER)
+      return fail(CATAPULT_EUNSUPPORTED, "the shear Alfven wave is built for Boozer tracing only");
+    if (!(std::isfinite(p->saw_omega) && p->saw_omega != 0.0 && std::isfinite(p->saw_w2) && p->saw_w2 > 0.0 &&
+          std::isfinite(p->saw_Phi0) && std::isfinite(p->saw_s0)))
+      return fail(CATAPULT_EINVAL, "saw_omega must be non-zero, saw_w2 > 0, saw_Phi0/saw_s0 finite");
+  }
+  tc->f = f->fc;
+  tc->M = p->mass;
+  tc->q = p->charge;
+  tc->Moq = p->mass / p->charge;
+  tc->vtot = std::sqrt(2.0 * p->energy / p->mass);
+  tc->vtot2 = tc->vtot * tc->vtot;
+  tc->T = p->T;
+  tc->rtol = p->rtol;
+  tc->atol = p->atol;
+  // DESIGN.md S3 defaults: dtmax = (pi/2) L / v_total, dt0 = 1e-3 dtmax
+  double dtmax = p->dtmax;
+  if (!(dtmax > 0.0)) {
+    double L;
+    if (f->desc.coord == CATAPULT_COORD_BOOZER) {
+      double b00 = 1.0;  // |B| at the first node = first coefficient of the first cell
+      cudaError_t e = cudaMemcpy(&b00, f->d_table, sizeof(double), cudaMemcpyDeviceToHost);
+      if (e != cudaSuccess) return cuda_fail(e, "reading |B|(node 0) for the default dtmax");
+      L = std::fabs(f->desc.G0) / std::fabs(b00);
+    } else {
+      L = f->desc.hi[0];
+    }
+    dtmax = 0.5 * PI * L / tc->vtot;
+  }
+  double dt0 = p->dt0 > 0.0 ? p->dt0 : 1e-3 * dtmax;
+  if (dt0 > dtmax) dt0 = dtmax;
+  tc->dt0 = dt0;
+  tc->dtmax = dtmax;
+  tc->max_steps = p->max_steps;
+  tc->max_rej = p->max_consecutive_rejects > 0 ? p->max_consecutive_rejects : 500;
+  tc->saw_m = p->saw_m;
+  tc->saw_n = p->saw_n;
+  tc->saw_Phi0 = p->saw_Phi0;
+  tc->saw_s0 = p->saw_s0;
+  tc->saw_invw2 = p->saw_on ? 1.0 / p->saw_w2 : 0.0;
+  tc->saw_omega = p->saw_omega;
+  *model = f->desc.coord == CATAPULT_COORD_CYL ? MODEL_CART : (p->saw_on ? MODEL_BOOZER_SAW : MODEL_BOOZER_VAC);
+  (void)E_CHARGE;
+  return CATAPULT_OK;
+}
+
+static catapult_status use_device_of(const catapult_field* f) {
+  int dev = -1;
+  CATAPULT_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev != f->device) return fail(CATAPULT_EINVAL, "field was built on another device than the current one");
+  return CATAPULT_OK;
+}
+
+}  // namespace catapult
+
+using namespace catapult;
+
+extern "C" {
+
+const char* catapult_last_error(void) { return g_last_error.c_str(); }
+const char* catapult_version(void) { return "catapult-b200 0.1 (sm_100a)"; }
+
+catapult_status catapult_field_build(const catapult_field_desc* desc, const double* d_nodes, void* stream,
+                                     catapult_field** out) {
+  catapult_status st = validate_desc(desc);
+  if (st != CATAPULT_OK) return st;
+  if (!d_nodes) return fail(CATAPULT_EINVAL, "d_nodes is NULL");
+  if (!out) return fail(CATAPULT_EINVAL, "out is NULL");
+  *out = nullptr;
+  catapult_field* f = new (std::nothrow) catapult_field();
+  if (!f) return fail(CATAPULT_ENOMEM, "host allocation failed");
+  f->desc = *desc;
+  f->ncells = (int64_t)desc->ncell[0] * desc->ncell[1] * desc->ncell[2];
+  f->table_bytes = (size_t)f->ncells * desc->nquant * 64 * sizeof(double);
+  f->d_table = nullptr;
+  cudaError_t e = cudaGetDevice(&f->device);
+  if (e == cudaSuccess) e = cudaMalloc((void**)&f->d_table, f->table_bytes);
+  if (e != cudaSuccess) {
+    delete f;
+    return cuda_fail(e, "cudaMalloc(table)");
+  }
+  fill_field_const(*desc, f->d_table, &f->fc);
+  st = launch_field_build(*desc, d_nodes, f->d_table, (cudaStream_t)stream);
+  if (st != CATAPULT_OK) {
+    cudaFree(f->d_table);
+    delete f;
+    return st;
+  }
+  *out = f;
+  return CATAPULT_OK;
+}
+
+catapult_status catapult_field_build_host(const catapult_field_desc* desc, const double* h_nodes,
+                                          catapult_field** out) {
+  catapult_status st = validate_desc(desc);
+  if (st != CATAPULT_OK) return st;
+  if (!h_nodes) return fail(CATAPULT_EINVAL, "h_nodes is NULL");
+  if (!out) return fail(CATAPULT_EINVAL, "out is NULL");
+  size_t nn = (size_t)desc->nquant;
+  for (int i = 0; i < 3; ++i) nn *= (size_t)(3 * desc->ncell[i] + 1);
+  double* d_nodes = nullptr;
+  CATAPULT_CUDA_TRY(cudaMalloc((void**)&d_nodes, nn * sizeof(double)));
+  cudaError_t e = cudaMemcpy(d_nodes, h_nodes, nn * sizeof(double), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    cudaFree(d_nodes);
+    return cuda_fail(e, "cudaMemcpy(nodes)");
+  }
+  st = catapult_field_build(desc, d_nodes, nullptr, out);
+  e = cudaDeviceSynchronize();
+  cudaFree(d_nodes);
+  if (st == CATAPULT_OK && e != cudaSuccess) {
+    catapult_field_destroy(*out);
+    *out = nullptr;
+    return cuda_fail(e, "field build");
+  }
+  return st;
+}
+
+catapult_status catapult_field_destroy(catapult_field* f) {
+  if (!f) return CATAPULT_OK;
+  if (f->d_table) cudaFree(f->d_table);
+  delete f;
+  return CATAPULT_OK;
+}
+
+size_t catapult_field_table_bytes(const catapult_field* f) { return f ? f->table_bytes : 0; }
+
+catapult_status catapult_field_eval(const catapult_field* f, int64_t npts, const double* d_pts, double* d_out,
+                                    void* stream) {
+  if (!f) return fail(CATAPULT_EINVAL, "field is NULL");
+  if (npts < 0) return fail(CATAPULT_EINVAL, "npts < 0");
+  if (npts > 0 && (!d_pts || !d_out)) return fail(CATAPULT_EINVAL, "d_pts/d_out is NULL");
+  catapult_status st = use_device_of(f);
+  if (st != CATAPULT_OK) return st;
+  return launch_field_eval(f->fc, npts, d_pts, d_out, (cudaStream_t)stream);
+}
+
+catapult_status catapult_field_export_rows(const catapult_field* f, double* d_out, void* stream) {
+  if (!f || !d_out) return fail(CATAPULT_EINVAL, "field/d_out is NULL");
+  catapult_status st = use_device_of(f);
+  if (st != CATAPULT_OK) return st;
+  return launch_field_export_rows(f->fc, f->ncells, d_out, (cudaStream_t)stream);
+}
+
+static catapult_status run_trace(const catapult_field* f, const catapult_trace_params* p, TraceArgs a,
+                                 cudaStream_t s) {
+  TraceConst tc;
+  int model = 0;
+  catapult_status st = make_trace_const(f, p, &tc, &model);
+  if (st != CATAPULT_OK) return st;
+  st = use_device_of(f);
+  if (st != CATAPULT_OK) return st;
+  if (a.n == 0) return CATAPULT_OK;
+  unsigned long long* queue = nullptr;
+  CATAPULT_CUDA_TRY(cudaMallocAsync((void**)&queue, sizeof(unsigned long long), s));
+  cudaError_t e = cudaMemsetAsync(queue, 0, sizeof(unsigned long long), s);
+  if (e != cudaSuccess) {
+    cudaFreeAsync(queue, s);
+    return cuda_fail(e, "cudaMemsetAsync(queue)");
+  }
+  a.queue = queue;
+  st = launch_trace(tc, a, model, s);
+  cudaFreeAsync(queue, s);
+  return st;
+}
+
+catapult_status catapult_trace(const catapult_field* f, const catapult_trace_params* p, int64_t n, const double* d_x0,
+                               double* d_xf, double* d_tstop, int32_t* d_status, uint32_t* d_nacc, uint32_t* d_nrej,
+                               uint64_t* d_counters, void* stream) {
+  if (n < 0) return fail(CATAPULT_EINVAL, "n < 0");
+  if (n > 0 && (!d_x0 || !d_xf || !d_tstop || !d_status))
+    return fail(CATAPULT_EINVAL, "d_x0, d_xf, d_tstop and d_status are required");
+  TraceArgs a{};
+  a.n = n;
+  a.x_in = d_x0;
+  a.x_out = d_xf;
+  a.t_io = d_tstop;
+  a.status = d_status;
+  a.nacc = d_nacc;
+  a.nrej = d_nrej;
+  a.counters = (unsigned long long*)d_counters;
+  return run_trace(f, p, a, (cudaStream_t)stream);
+}
+
+catapult_status catapult_trace_init(const catapult_field* f, const catapult_trace_params* p, int64_t n,
+                                    const double* d_x, double* d_t, double* d_dt, double* d_mu, int32_t* d_status,
+                                    void* stream) {
+  if (n < 0) return fail(CATAPULT_EINVAL, "n < 0");
+  if (n > 0 && (!d_x || !d_t || !d_dt || !d_mu || !d_status))
+    return fail(CATAPULT_EINVAL, "d_x, d_t, d_dt, d_mu and d_status are required");
+  TraceArgs a{};
+  a.n = n;
+  a.x_in = d_x;
+  a.x_out = const_cast<double*>(d_x);  // only rewritten (unchanged) for particles born outside
+  a.t_io = d_t;
+  a.dt_io = d_dt;
+  a.mu_io = d_mu;
+  a.status = d_status;
+  a.init_only = 1;
+  return run_trace(f, p, a, (cudaStream_t)stream);
+}
+
+catapult_status catapult_trace_continue(const catapult_field* f, const catapult_trace_params* p, int64_t n,
+                                        double* d_x, double* d_t, double* d_dt, double* d_mu, int32_t* d_status,
+                                        uint32_t* d_nacc, uint32_t* d_nrej, uint64_t* d_counters, void* stream) {
+  if (n < 0) return fail(CATAPULT_EINVAL, "n < 0");
+  if (n > 0 && (!d_x || !d_t || !d_dt || !d_mu || !d_status))
+    return fail(CATAPULT_EINVAL, "d_x, d_t, d_dt, d_mu and d_status are required");
+  TraceArgs a{};
+  a.n = n;
+  a.x_in = d_x;
+  a.x_out = d_x;
+  a.t_io = d_t;
+  a.dt_io = d_dt;
+  a.mu_io = d_mu;
+  a.status = d_status;
+  a.nacc = d_nacc;
+  a.nrej = d_nrej;
+  a.counters = (unsigned long long*)d_counters;
+  a.resume = 1;
+  return run_trace(f, p, a, (cudaStream_t)stream);
+}
+
+catapult_status catapult_trace_host(const catapult_field* f, const catapult_trace_params* p, int64_t n,
+                                    const double* h_x0, double* h_xf, double* h_tstop, int32_t* h_status,
+                                    uint32_t* h_nacc, uint32_t* h_nrej, uint64_t* h_counters) {
+  if (n < 0) return fail(CATAPULT_EINVAL, "n < 0");
+  if (n > 0 && (!h_x0 || !h_xf || !h_tstop || !h_status))
+    return fail(CATAPULT_EINVAL, "h_x0, h_xf, h_tstop and h_status are required");
+  if (!f || !p) return fail(CATAPULT_EINVAL, "field/params is NULL");
+  if (n == 0) return CATAPULT_OK;
+  // one device slab: x0[4n] xf[4n] tstop[n] | status[n] nacc[n] nrej[n] | counters[8]
+  const size_t nd = (size_t)n;
+  const size_t bytes = nd * 9 * sizeof(double) + nd * 3 * sizeof(uint32_t) + 8 * sizeof(uint64_t) + 64;
+  char* slab = nullptr;
+  CATAPULT_CUDA_TRY(cudaMalloc((void**)&slab, bytes));
+  double* d_x0 = (double*)slab;
+  double* d_xf = d_x0 + 4 * nd;
+  double* d_ts = d_xf + 4 * nd;
+  uint64_t* d_cnt = (uint64_t*)(d_ts + nd);
+  int32_t* d_st = (int32_t*)(d_cnt + 8);
+  uint32_t* d_na = (uint32_t*)(d_st + nd);
+  uint32_t* d_nr = d_na + nd;
+  catapult_status st = CATAPULT_OK;
+  cudaError_t e = cudaMemcpyAsync(d_x0, h_x0, 4 * nd * sizeof(double), cudaMemcpyHostToDevice, 0);
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_cnt, 0, 8 * sizeof(uint64_t), 0);
+  if (e == cudaSuccess) {
+    st = catapult_trace(f, p, n, d_x0, d_xf, d_ts, d_st, d_na, d_nr, d_cnt, nullptr);
+    if (st == CATAPULT_OK) {
+      e = cudaMemcpyAsync(h_xf, d_xf, 4 * nd * sizeof(double), cudaMemcpyDeviceToHost, 0);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h_tstop, d_ts, nd * sizeof(double), cudaMemcpyDeviceToHost, 0);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h_status, d_st, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, 0);
+      if (e == cudaSuccess && h_nacc)
+        e = cudaMemcpyAsync(h_nacc, d_na, nd * sizeof(uint32_t), cudaMemcpyDeviceToHost, 0);
+      if (e == cudaSuccess && h_nrej)
+        e = cudaMemcpyAsync(h_nrej, d_nr, nd * sizeof(uint32_t), cudaMemcpyDeviceToHost, 0);
+      if (e == cudaSuccess && h_counters)
+        e = cudaMemcpyAsync(h_counters, d_cnt, 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost, 0);
+    }
+  }
+  cudaError_t e2 = cudaStreamSynchronize(0);
+  cudaFree(slab);
+  if (st != CATAPULT_OK) return st;
+  if (e != cudaSuccess) return cuda_fail(e, "catapult_trace_host copies");
+  if (e2 != cudaSuccess) return cuda_fail(e2, "catapult_trace_host");
+  return CATAPULT_OK;
+}
+
+catapult_status catapult_trace_continue_host(const catapult_field* f, const catapult_trace_params* p, int64_t n,
+                                             double* h_x, double* h_t, double* h_dt, double* h_mu, int32_t* h_status,
+                                             uint32_t* h_nacc, uint32_t* h_nrej, uint64_t* h_counters) {
+  if (n < 0) return fail(CATAPULT_EINVAL, "n < 0");
+  if (n > 0 && (!h_x || !h_t || !h_dt || !h_mu || !h_status))
+    return fail(CATAPULT_EINVAL, "h_x, h_t, h_dt, h_mu and h_status are required");
+  if (!f || !p) return fail(CATAPULT_EINVAL, "field/params is NULL");
+  if (n == 0) return CATAPULT_OK;
+  // one device slab: x[4n] t[n] dt[n] mu[n] | counters[8] | status[n] nacc[n] nrej[n]
+  const size_t nd = (size_t)n;
+  const size_t bytes = nd * 7 * sizeof(double) + 8 * sizeof(uint64_t) + nd * 3 * sizeof(uint32_t) + 64;
+  char* slab = nullptr;
+  CATAPULT_CUDA_TRY(cudaMalloc((void**)&slab, bytes));
+  double* d_x = (double*)slab;
+  double* d_t = d_x + 4 * nd;
+  double* d_dt = d_t + nd;
+  double* d_mu = d_dt + nd;
+  uint64_t* d_cnt = (uint64_t*)(d_mu + nd);
+  int32_t* d_st = (int32_t*)(d_cnt + 8);
+  uint32_t* d_na = (uint32_t*)(d_st + nd);
+  uint32_t* d_nr = d_na + nd;
+  catapult_status st = CATAPULT_OK;
+  const cudaMemcpyKind H2D = cudaMemcpyHostToDevice, D2H = cudaMemcpyDeviceToHost;
+  cudaError_t e = cudaMemcpyAsync(d_x, h_x, 4 * nd * sizeof(double), H2D, 0);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_t, h_t, nd * sizeof(double), H2D, 0);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_dt, h_dt, nd * sizeof(double), H2D, 0);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_mu, h_mu, nd * sizeof(double), H2D, 0);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_st, h_status, nd * sizeof(int32_t), H2D, 0);
+  if (e == cudaSuccess) e = h_nacc ? cudaMemcpyAsync(d_na, h_nacc, nd * sizeof(uint32_t), H2D, 0)
+                                   : cudaMemsetAsync(d_na, 0, nd * sizeof(uint32_t), 0);
+  if (e == cudaSuccess) e = h_nrej ? cudaMemcpyAsync(d_nr, h_nrej, nd * sizeof(uint32_t), H2D, 0)
+                                   : cudaMemsetAsync(d_nr, 0, nd * sizeof(uint32_t), 0);
+  if (e == cudaSuccess) e = h_counters ? cudaMemcpyAsync(d_cnt, h_counters, 8 * sizeof(uint64_t), H2D, 0)
+                                       : cudaMemsetAsync(d_cnt, 0, 8 * sizeof(uint64_t), 0);
+  if (e == cudaSuccess) {
+    st = catapult_trace_continue(f, p, n, d_x, d_t, d_dt, d_mu, d_st, d_na, d_nr, d_cnt, nullptr);
+    if (st == CATAPULT_OK) {
+      e = cudaMemcpyAsync(h_x, d_x, 4 * nd * sizeof(double), D2H, 0);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h_t, d_t, nd * sizeof(double), D2H, 0);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h_dt, d_dt, nd * sizeof(double), D2H, 0);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h_mu, d_mu, nd * sizeof(double), D2H, 0);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h_status, d_st, nd * sizeof(int32_t), D2H, 0);
+      if (e == cudaSuccess && h_nacc) e = cudaMemcpyAsync(h_nacc, d_na, nd * sizeof(uint32_t), D2H, 0);
+      if (e == cudaSuccess && h_nrej) e = cudaMemcpyAsync(h_nrej, d_nr, nd * sizeof(uint32_t), D2H, 0);
+      if (e == cudaSuccess && h_counters) e = cudaMemcpyAsync(h_counters, d_cnt, 8 * sizeof(uint64_t), D2H, 0);
+    }
+  }
+  cudaError_t e2 = cudaStreamSynchronize(0);
+  cudaFree(slab);
+  if (st != CATAPULT_OK) return st;
+  if (e != cudaSuccess) return cuda_fail(e, "catapult_trace_continue_host copies");
+  if (e2 != cudaSuccess) return cuda_fail(e2, "catapult_trace_continue_host");
+  return CATAPULT_OK;
+}
+
+catapult_status catapult_step_once(const catapult_field* f, const catapult_trace_params* p, int64_t n,
+                                   const double* d_x, const double* d_t, const double* d_h, double* d_xnew,
+                                   double* d_errratio, double* d_k, void* stream) {
+  if (n < 0) return fail(CATAPULT_EINVAL, "n < 0");
+  if (n > 0 && (!d_x || !d_t || !d_h || !d_xnew || !d_errratio || !d_k))
+    return fail(CATAPULT_EINVAL, "all array arguments of catapult_step_once are required");
+  TraceConst tc;
+  int model = 0;
+  catapult_status st = make_trace_const(f, p, &tc, &model);
+  if (st != CATAPULT_OK) return st;
+  st = use_device_of(f);
+  if (st != CATAPULT_OK) return st;
+  return launch_step_once(tc, model, n, d_x, d_t, d_h, d_xnew, d_errratio, d_k, (cudaStream_t)stream);
+}
+
+catapult_status catapult_estimate(int32_t g_kind, int64_t n, const int32_t* d_status, const double* d_tstop,
+                                  const double* d_g_user, double* d_out, double* h_out, void* stream) {
+  if (n < 0) return fail(CATAPULT_EINVAL, "n < 0");
+  if (g_kind < 0 || g_kind > 2) return fail(CATAPULT_EINVAL, "g_kind must be 0, 1 or 2");
+  if (!d_out) return fail(CATAPULT_EINVAL, "d_out is NULL");
+  if (n > 0 && ((g_kind == 0 && !d_status) || (g_kind == 1 && !d_tstop) || (g_kind == 2 && !d_g_user)))
+    return fail(CATAPULT_EINVAL, "the array selected by g_kind is NULL");
+  catapult_status st = launch_estimate(g_kind, n, d_status, d_tstop, d_g_user, d_out, (cudaStream_t)stream);
+  if (st != CATAPULT_OK) return st;
+  if (h_out) {
+    CATAPULT_CUDA_TRY(cudaMemcpyAsync(h_out, d_out, 3 * sizeof(double), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CATAPULT_CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+  }
+  return CATAPULT_OK;
+}
+
+catapult_status catapult_measure_fp64_peak(double* flops_per_s) {
+  if (!flops_per_s) return fail(CATAPULT_EINVAL, "flops_per_s is NULL");
+  return measure_fp64_peak(flops_per_s);
+}
+
+catapult_status catapult_measure_l2_bandwidth(size_t bytes, double* bytes_per_s) {
+  if (!bytes_per_s) return fail(CATAPULT_EINVAL, "bytes_per_s is NULL");
+  return measure_l2_bandwidth(bytes, bytes_per_s);
+}
+
+catapult_status catapult_trace_launch_shape(const catapult_field* f, const catapult_trace_params* p, int32_t* blocks,
+                                            int32_t* threads) {
+  if (!blocks || !threads) return fail(CATAPULT_EINVAL, "blocks/threads is NULL");
+  TraceConst tc;
+  int model = 0;
+  catapult_status st = make_trace_const(f, p, &tc, &model);
+  if (st != CATAPULT_OK) return st;
+  int b = 0, t = 0;
+  st = trace_launch_shape(model, (int64_t)1 << 40, &b, &t);
+  *blocks = b;
+  *threads = t;
+  return st;
+}
+
+}  // extern "C"

@@ -1,0 +1,89 @@
+// Internal declarations shared by the translation units of libcatapult.so (not installed).
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <string>
+
+#include "catapult.h"
+
+namespace catapult {
+
+// Field geometry + profile parameters as the kernels see them.  Passed by value as a
+// __grid_constant__ kernel parameter, i.e. it lives in the constant bank (PAPER.md:65:
+// "Data that is used by all threads is moved to constant memory").
+struct FieldConst {
+  const double* table;  // [cell][quantity][64], cell-major (include/catapult.h)
+  int coord, m;
+  int k[3];
+  double lo[3], invh[3], span[3], invspan[3];
+  double G, invG, psi0, invpsi0, iota0, iota1;
+};
+
+struct TraceConst {
+  FieldConst f;
+  double M, q, Moq, vtot, vtot2;
+  double T, rtol, atol, dt0, dtmax;
+  long long max_steps;
+  int max_rej;
+  int saw_m, saw_n;
+  double saw_Phi0, saw_s0, saw_invw2, saw_omega;
+};
+
+struct TraceArgs {
+  long long n;
+  const double* x_in;  // [4][n]
+  double* x_out;       // [4][n]
+  double* t_io;        // [n]; in only when resume
+  double* dt_io;       // [n] or nullptr
+  double* mu_io;       // [n] or nullptr
+  int* status;         // [n]; in only when resume
+  unsigned* nacc;      // nullable
+  unsigned* nrej;      // nullable
+  unsigned long long* counters;  // nullable, 8 entries
+  unsigned long long* queue;     // work counter, zero at launch
+  int resume;     // 1: continue from (t,dt,mu,status) arrays
+  int init_only;  // 1: only fill (t,dt,mu,status)
+};
+
+void set_error(const std::string& msg);
+catapult_status cuda_fail(cudaError_t e, const char* what);
+
+#define CATAPULT_CUDA_TRY(expr)                                        \
+  do {                                                                 \
+    cudaError_t _e = (expr);                                           \
+    if (_e != cudaSuccess) return ::catapult::cuda_fail(_e, #expr);    \
+  } while (0)
+
+// field.cu
+catapult_status launch_field_build(const catapult_field_desc& d, const double* d_nodes, double* d_table,
+                                   cudaStream_t s);
+catapult_status launch_field_eval(const FieldConst& fc, int64_t npts, const double* d_pts, double* d_out,
+                                  cudaStream_t s);
+catapult_status launch_field_export_rows(const FieldConst& fc, int64_t ncells, double* d_out, cudaStream_t s);
+
+// tracer.cu
+catapult_status launch_trace(const TraceConst& tc, const TraceArgs& a, int model, cudaStream_t s);
+catapult_status launch_step_once(const TraceConst& tc, int model, int64_t n, const double* d_x, const double* d_t,
+                                 const double* d_h, double* d_xnew, double* d_err, double* d_k, cudaStream_t s);
+catapult_status trace_launch_shape(int model, int64_t n, int* blocks, int* threads);
+
+// estimate.cu
+catapult_status launch_estimate(int g_kind, int64_t n, const int* d_status, const double* d_tstop,
+                                const double* d_g, double* d_out, cudaStream_t s);
+
+// peaks.cu
+catapult_status measure_fp64_peak(double* flops);
+catapult_status measure_l2_bandwidth(size_t bytes, double* bps);
+
+}  // namespace catapult
+
+struct catapult_field {
+  catapult_field_desc desc;
+  catapult::FieldConst fc;
+  double* d_table;
+  size_t table_bytes;
+  int64_t ncells;
+  int device;
+};

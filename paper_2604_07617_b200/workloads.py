@@ -200,24 +200,30 @@ FULL_NCELL = [[16, 16, 16], [16, 16, 16], [64, 64, 64], [48, 48, 32], [64, 64, 6
 
 
 def config(idx: int, n: int | None = None, T: float | None = None, ncell=None,
-           with_nodes: bool = True) -> dict:
+           with_nodes: bool = True, ensemble: int = 0) -> dict:
     """Returns dict(name, field, params, x0, g_kind).  n/T/ncell override the full sizes (parity
-    tests run reduced sizes of the same recipe; the first n particles of the seeded stream)."""
+    tests run reduced sizes of the same recipe; the first n particles of the seeded stream).
+    ensemble > 0 draws an independent birth ensemble of the same distribution (seed [seed, ensemble]):
+    used only to give every rank of a multi-GPU weak-scaling run its own particles."""
     idx = int(idx)
+
+    def _rng(seed):
+        return np.random.default_rng(seed if ensemble == 0 else [seed, int(ensemble)])
+
     nfull = FULL_N[idx]
     n = nfull if n is None else int(n)
     T = FULL_T[idx] if T is None else float(T)
     ncell = FULL_NCELL[idx] if ncell is None else [int(v) for v in ncell]
     if idx in (0, 1):
         modes = boozer_modes_cfg0()
-        rng = np.random.default_rng(idx)
+        rng = _rng(idx)
         x0 = boozer_births(rng, max(n, nfull), s_fixed=0.25)[:, :n]
         params = base_params(T)
         field = boozer_field(modes, ncell) if with_nodes else None
     elif idx in (2, 4):
         rng2 = np.random.default_rng(2)
         modes = boozer_modes_random(rng=rng2)
-        prng = rng2 if idx == 2 else np.random.default_rng(4)
+        prng = (rng2 if ensemble == 0 else _rng(2)) if idx == 2 else _rng(4)
         x0 = boozer_births(prng, max(n, nfull), s_range=(0.1, 0.9))[:, :n]
         params = base_params(T)
         if idx == 4:
@@ -225,7 +231,7 @@ def config(idx: int, n: int | None = None, T: float | None = None, ncell=None,
                           saw_omega=2.0 * math.pi * 1.0e5)
         field = boozer_field(modes, ncell) if with_nodes else None
     elif idx == 3:
-        rng = np.random.default_rng(3)
+        rng = _rng(3)
         x0 = cyl_births(rng, max(n, nfull))[:, :n]
         field = cyl_field(ncell) if with_nodes else None
         params = base_params(T, L=R0 + 1.25 * A_MINOR)

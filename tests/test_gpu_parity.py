@@ -1,0 +1,359 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle on the same seeded
+inputs.  Tolerances are BASELINE.json north_star's (restated in DESIGN.md "Tolerances"):
+  field values / derivatives   1e-12 relative to the column's max-abs (reading Q11)
+  one attempted step           1e-11
+  trajectories over 1e-5 s     1e-8 relative
+  loss fraction                3 binomial standard deviations at n >= 1e4
+  table rows / statuses / counts: bit-exact where unique.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from paper_2604_07617_b200 import workloads as W  # noqa: E402
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+@pytest.fixture(scope="module")
+def K():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    from paper_2604_07617_b200 import binding
+    binding.load()
+    return binding
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _state_scale(coord):
+    return np.array([1.0, 1.0, 1.0, W.V_TOTAL]) if coord == 0 else np.array([W.R0, W.R0, W.R0, W.V_TOTAL])
+
+
+def _state_diff(coord, a, b):
+    d = a - b
+    if coord == 0:
+        d[1] = np.remainder(d[1] + math.pi, 2 * math.pi) - math.pi
+    return d
+
+
+SMALL = {  # reduced sizes of the five recipes: several cells per dim, ragged particle counts
+    0: dict(n=64, T=1e-5),
+    1: dict(n=77, T=1e-5),
+    2: dict(n=45, T=1e-5, ncell=[12, 10, 9]),
+    3: dict(n=50, T=1e-5, ncell=[12, 11, 5]),
+    4: dict(n=33, T=1e-5, ncell=[12, 10, 9]),
+}
+
+
+@pytest.fixture(scope="module")
+def cases(K, oracle):
+    out = {}
+    for idx, kw in SMALL.items():
+        cfg = W.config(idx, **kw)
+        out[idx] = dict(cfg=cfg, gf=K.catapult_field_build(cfg["field"]), of=oracle.Field(cfg["field"]),
+                        op=oracle.make_params(cfg["params"]))
+    return out
+
+
+# ---- a1: field build ---------------------------------------------------------------------------
+@pytest.mark.parametrize("idx", [0, 2, 3])
+def test_field_build_rows_bit_exact(K, oracle, cases, idx):
+    c = cases[idx]
+    rows = K.catapult_field_export_rows(c["gf"]).cpu().numpy()
+    want = oracle.field_build(c["of"])
+    assert rows.shape == want.shape
+    assert np.array_equal(rows, want)
+    assert c["gf"].table_bytes == want.size * 8
+
+
+def test_field_build_host_equals_device_build(K, cases):
+    cfg = cases[3]["cfg"]
+    fh = K.catapult_field_build_host(cfg["field"])
+    a = K.catapult_field_export_rows(fh)
+    b = K.catapult_field_export_rows(cases[3]["gf"])
+    assert torch.equal(a, b)
+
+
+# ---- a4/a5: locate + tricubic ----------------------------------------------------------------------
+@pytest.mark.parametrize("idx", [0, 2, 3])
+def test_field_eval_parity(K, oracle, cases, idx):
+    c = cases[idx]
+    fd = c["cfg"]["field"]
+    rng = np.random.default_rng(100 + idx)
+    npts = 4099
+    pts = np.zeros((3, npts))
+    for d in range(3):
+        span = fd["hi"][d] - fd["lo"][d]
+        pts[d] = fd["lo"][d] + span * rng.random(npts)
+    # extrapolation in dim 0 (s > 1, s < 0), wrap-around in the periodic dims, exact faces and edges
+    pts[0, :200] = fd["hi"][0] + 0.2 * (fd["hi"][0] - fd["lo"][0]) * rng.random(200)
+    pts[0, 200:300] = fd["lo"][0] - 0.05 * rng.random(100)
+    pts[2, 300:600] += (fd["hi"][2] - fd["lo"][2]) * rng.integers(-5, 6, size=300)
+    if fd["coord"] == 0:
+        pts[1, 600:900] += 2 * math.pi * rng.integers(-3, 4, size=300)
+    else:
+        pts[1, 600:700] = fd["hi"][1] + 0.3 * rng.random(100)
+    h0 = (fd["hi"][0] - fd["lo"][0]) / fd["ncell"][0]
+    pts[0, 900:900 + fd["ncell"][0] + 1] = fd["lo"][0] + h0 * np.arange(fd["ncell"][0] + 1)
+    pts[2, 950] = fd["hi"][2]
+    pts[2, 951] = fd["lo"][2]
+    got = K.catapult_field_eval(c["gf"], _dev(pts)).cpu().numpy()
+    want = oracle.tricubic_many(c["of"], pts)
+    scale = np.abs(fd["nodes"]).reshape(fd["nquant"], -1).max(axis=1)
+    scale = np.where(scale > 0, scale, 1.0)
+    err = np.abs(got - want) / scale[:, None]
+    # extrapolated points amplify round-off by the size of the basis polynomials (|L| up to ~30 at u=2)
+    assert err[:, 300:].max() < 1e-12, err[:, 300:].max()
+    assert err[:, :300].max() < 5e-11, err[:, :300].max()
+
+
+# ---- a3-a7: one attempted step from identical state ------------------------------------------------
+@pytest.mark.parametrize("idx", [0, 2, 3, 4])
+def test_single_step_parity(K, oracle, cases, idx):
+    c = cases[idx]
+    cfg = c["cfg"]
+    x0 = cfg["x0"]
+    n = x0.shape[1]
+    rng = np.random.default_rng(200 + idx)
+    t = 1e-6 * rng.random(n)
+    h = cfg["params"]["dtmax"] * (0.02 + 0.1 * rng.random(n))
+    xg, rg, kg = K.catapult_step_once(c["gf"], cfg["params"], _dev(x0), _dev(t), _dev(h))
+    xg, rg, kg = xg.cpu().numpy(), rg.cpu().numpy(), kg.cpu().numpy()
+    sc = _state_scale(cfg["field"]["coord"])
+    for i in range(n):
+        xo, ro, ko = oracle.step_once(c["of"], c["op"], x0[:, i], t[i], h[i])
+        d = _state_diff(cfg["field"]["coord"], xg[:, i], xo)
+        assert np.all(np.abs(d) <= 1e-11 * sc), (i, d)
+        kscale = np.abs(ko).max(axis=0)
+        assert np.all(np.abs(kg[:, :, i] - ko) <= 1e-11 * kscale[None, :] + 1e-300), (i,)
+        # the error ratio is a quotient of a cancellation-prone difference: compare loosely
+        assert abs(rg[i] - ro) <= 1e-3 * max(ro, 1e-3), (i, rg[i], ro)
+
+
+# ---- whole trajectories over the 1e-5 s window ----------------------------------------------------
+@pytest.mark.parametrize("idx", [0, 1, 2, 3, 4])
+def test_trajectory_parity_1e5_window(K, oracle, cases, idx):
+    c = cases[idx]
+    cfg = c["cfg"]
+    g = K.catapult_trace(c["gf"], cfg["params"], _dev(cfg["x0"]))
+    o = oracle.trace(c["of"], c["op"], cfg["x0"])
+    gs = g["status"].cpu().numpy()
+    assert np.array_equal(gs, o["status"])
+    gx, gt = g["xf"].cpu().numpy(), g["tstop"].cpu().numpy()
+    sc = _state_scale(cfg["field"]["coord"])
+    d = _state_diff(cfg["field"]["coord"], gx, o["xf"])
+    assert np.all(np.abs(d) <= 1e-8 * np.maximum(sc[:, None], np.abs(o["xf"]))), np.abs(d).max(axis=1)
+    assert np.allclose(gt, o["tstop"], rtol=1e-9, atol=0)
+    alive = gs == 0
+    assert np.all(gt[alive] == cfg["params"]["T"])
+    # step counts are integers decided by floating point: identical except where r sits at a threshold
+    na, nr = g["nacc"].cpu().numpy(), g["nrej"].cpu().numpy()
+    assert np.mean(na == o["nacc"]) > 0.9 and np.mean(nr == o["nrej"]) > 0.9
+    assert np.abs(na.astype(int) - o["nacc"].astype(int)).max() <= 3
+    cnt = g["counters"].cpu().numpy()
+    assert cnt[0] == na.sum() and cnt[1] == nr.sum()
+    assert cnt[2] == np.sum(gs == 0) and cnt[3] == np.sum(gs == 1)
+    assert cnt[6] >= 6 * (na.sum() + nr.sum())
+
+
+def test_cfg0_full_statistics(K, oracle):
+    """Config 0 at full size (64 alphas, T = 1e-4 s): beyond 1e-5 s orbits are compared statistically
+    (reading Q13) -- statuses, loss times and energy drift distribution."""
+    cfg = W.config(0)
+    gf = K.catapult_field_build(cfg["field"])
+    of, op = oracle.Field(cfg["field"]), oracle.make_params(cfg["params"])
+    g = K.catapult_trace(gf, cfg["params"], _dev(cfg["x0"]))
+    o = oracle.trace(of, op, cfg["x0"])
+    gs = g["status"].cpu().numpy()
+    assert np.mean(gs == o["status"]) >= 0.95
+    both_lost = (gs == 1) & (o["status"] == 1)
+    assert np.allclose(g["tstop"].cpu().numpy()[both_lost], o["tstop"][both_lost], rtol=1e-3)
+    # energy drift (reading Q3): interpolation-limited, identical distribution on both sides
+    x0 = cfg["x0"]
+
+    def drift(xf):
+        B0v = oracle.tricubic_many(of, x0[:3])[0]
+        Bf = oracle.tricubic_many(of, xf[:3])[0]
+        mu = (W.V_TOTAL ** 2 - x0[3] ** 2) / (2 * B0v)
+        return np.abs((0.5 * xf[3] ** 2 + mu * Bf) / (0.5 * W.V_TOTAL ** 2) - 1)
+
+    keep = (gs == 0) & (o["status"] == 0)
+    dg, do = drift(g["xf"].cpu().numpy())[keep], drift(o["xf"])[keep]
+    assert np.median(dg) < 5e-6 and abs(np.median(dg) - np.median(do)) < 0.2 * np.median(do) + 1e-9
+    na = g["nacc"].cpu().numpy()
+    assert abs(na.sum() / o["nacc"].sum() - 1) < 0.01
+
+
+def test_cfg1_loss_fraction_within_3_sigma(K):
+    """Config 1 at full size (10,000 alphas, T = 1e-3 s, launch shape of bench.py) against the oracle's
+    stored result (tests/golden/cfg1_oracle.txt, written by tests/golden/make_golden.py from oracle/)."""
+    path = os.path.join(GOLDEN, "cfg1_oracle.txt")
+    if not os.path.exists(path):
+        pytest.fail("tests/golden/cfg1_oracle.txt missing: run python tests/golden/make_golden.py")
+    gold = {}
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, v = line.split("=", 1)
+        gold[k.strip()] = v.strip()
+    n = int(gold["n"])
+    lost_o = np.array([int(ch) for ch in gold["lost_bits"]], dtype=np.int32)
+    cfg = W.config(1)
+    assert n == cfg["x0"].shape[1] == 10_000
+    gf = K.catapult_field_build(cfg["field"])
+    g = K.catapult_trace(gf, cfg["params"], _dev(cfg["x0"]))
+    est = K.catapult_estimate(0, d_status=g["status"])
+    p_o = lost_o.mean()
+    sigma = math.sqrt(p_o * (1 - p_o) / n)
+    assert abs(est[0] - p_o) <= 3 * sigma, (est[0], p_o, sigma)
+    gs = g["status"].cpu().numpy()
+    assert est[2] == np.sum(gs == 1)
+    # per-particle agreement is far better than binomial noise: most orbits are not near the edge
+    assert np.mean((gs == 1) == (lost_o == 1)) > 0.97
+    assert abs(g["nacc"].sum().item() / float(gold["nacc_sum"]) - 1) < 0.01
+
+
+# ---- invariants on the GPU result ------------------------------------------------------------------
+def test_cartesian_pphi_conserved_on_gpu(K, oracle, cases):
+    c = cases[3]
+    cfg = W.config(3, n=256, T=1e-4, ncell=[24, 24, 4])
+    gf = K.catapult_field_build(cfg["field"])
+    of = oracle.Field(cfg["field"])
+    g = K.catapult_trace(gf, cfg["params"], _dev(cfg["x0"]))
+    assert torch.all(g["status"] == 0)
+
+    def inv(x):
+        R = np.hypot(x[0], x[1])
+        v = oracle.tricubic_many(of, np.array([R, x[2], np.arctan2(x[1], x[0])]))
+        modB = np.sqrt(v[0] ** 2 + v[1] ** 2 + v[2] ** 2)
+        mu = None
+        return R, v, modB
+
+    x0, xf = cfg["x0"], g["xf"].cpu().numpy()
+    R0_, v0, B0_ = inv(x0)
+    R1_, v1, B1_ = inv(xf)
+    mu = (W.V_TOTAL ** 2 - x0[3] ** 2) / (2 * B0_)
+    E1 = 0.5 * xf[3] ** 2 + mu * B1_
+    assert np.max(np.abs(E1 / (0.5 * W.V_TOTAL ** 2) - 1)) < 1e-6
+    P0 = W.ALPHA_MASS * R0_ * v0[1] / B0_ * x0[3] + W.ALPHA_CHARGE * v0[6]
+    P1 = W.ALPHA_MASS * R1_ * v1[1] / B1_ * xf[3] + W.ALPHA_CHARGE * v1[6]
+    assert np.max(np.abs(P1 - P0)) < 1e-6 * W.ALPHA_CHARGE * W.PSI_EDGE_CYL
+
+
+# ---- a9: stop logic, refill, restart ----------------------------------------------------------------
+def test_edge_cases(K, oracle, cases):
+    c = cases[0]
+    cfg = c["cfg"]
+    gf = c["gf"]
+    # n = 0
+    g = K.catapult_trace(gf, cfg["params"], torch.empty((4, 0), dtype=torch.float64, device="cuda"))
+    assert g["xf"].shape == (4, 0)
+    # born outside; one particle; max_steps; stall guard
+    x0 = cfg["x0"][:, :5].copy()
+    x0[0, 0] = 1.2
+    g = K.catapult_trace(gf, cfg["params"], _dev(x0))
+    assert g["status"][0].item() == 1 and g["tstop"][0].item() == 0.0
+    assert np.array_equal(g["xf"].cpu().numpy()[:, 0], x0[:, 0]) and g["nacc"][0].item() == 0
+    pd = dict(cfg["params"], max_steps=5)
+    g = K.catapult_trace(gf, pd, _dev(cfg["x0"]))
+    assert torch.all(g["status"] == 3) and torch.all(g["nacc"] + g["nrej"] == 5)
+    o = oracle.trace(c["of"], oracle.make_params(pd), cfg["x0"])
+    assert np.array_equal(g["nacc"].cpu().numpy(), o["nacc"])
+    pd = dict(cfg["params"], dt0=1e-3, dtmax=1e-3, max_consecutive_rejects=2)
+    g = K.catapult_trace(gf, pd, _dev(cfg["x0"]))
+    assert torch.all(g["status"] == 2) and torch.all(g["nrej"] == 2)
+    # bad parameters are rejected before any launch
+    with pytest.raises(K.CatapultError):
+        K.catapult_trace(gf, dict(cfg["params"], T=float("nan")), _dev(cfg["x0"]))
+    with pytest.raises(K.CatapultError):
+        K.catapult_trace(gf, dict(cfg["params"], rtol=0.0, atol=0.0), _dev(cfg["x0"]))
+    with pytest.raises(K.CatapultError):
+        K.catapult_trace(cases[3]["gf"], dict(cfg["params"], saw_on=1, saw_omega=1.0, saw_w2=0.1), _dev(cfg["x0"]))
+
+
+def test_refill_queue_many_more_particles_than_threads(K, oracle):
+    """More particles than resident threads with very uneven lifetimes: every index is traced exactly
+    once and matches a per-particle oracle run on a sample."""
+    b_cfg = W.config(1, n=10_000, T=2e-6)
+    gf = K.catapult_field_build(b_cfg["field"])
+    blocks, threads = K.catapult_trace_launch_shape(gf, b_cfg["params"])
+    reps = max(2, (3 * blocks * threads) // 10_000 + 1)
+    x0 = np.tile(b_cfg["x0"], (1, reps))
+    n = x0.shape[1]
+    assert n > 2 * blocks * threads
+    x0[0, ::7] = 1.5                       # born outside: finish at once
+    x0[0, 1::5] = 0.995                    # near the edge: many are lost early
+    g = K.catapult_trace(gf, b_cfg["params"], _dev(x0))
+    gs, gx = g["status"].cpu().numpy(), g["xf"].cpu().numpy()
+    assert np.all((gs == 0) | (gs == 1))
+    assert np.all(gs[::7] == 1) and np.array_equal(gx[:, ::7], x0[:, ::7])
+    # copies of the same particle give bit-identical results wherever they ran
+    base = 10_000
+    same = (x0[0, :base] == x0[0, base:2 * base])
+    assert np.array_equal(gx[:, :base][:, same], gx[:, base:2 * base][:, same])
+    of, op = oracle.Field(b_cfg["field"]), oracle.make_params(b_cfg["params"])
+    pick = np.random.default_rng(5).choice(n, size=64, replace=False)
+    o = oracle.trace(of, op, x0[:, pick])
+    assert np.array_equal(gs[pick], o["status"])
+    d = _state_diff(0, gx[:, pick], o["xf"])
+    assert np.all(np.abs(d) <= 1e-8 * np.array([1, 1, 1, W.V_TOTAL])[:, None])
+    cnt = g["counters"].cpu().numpy()
+    assert cnt[2] + cnt[3] == n
+
+
+def test_init_continue_equals_trace_and_windows(K, cases):
+    c = cases[2]
+    cfg = c["cfg"]
+    g = K.catapult_trace(c["gf"], cfg["params"], _dev(cfg["x0"]))
+    st = K.catapult_trace_init(c["gf"], cfg["params"], _dev(cfg["x0"]).clone())
+    K.catapult_trace_continue(c["gf"], cfg["params"], st)
+    assert torch.equal(st["x"], g["xf"]) and torch.equal(st["t"], g["tstop"]) and torch.equal(st["status"], g["status"])
+    assert torch.equal(st["nacc"], g["nacc"])
+    # two windows: same orbit up to the controller's restart at the window edge
+    st2 = K.catapult_trace_init(c["gf"], cfg["params"], _dev(cfg["x0"]).clone())
+    K.catapult_trace_continue(c["gf"], dict(cfg["params"], T=0.4e-5), st2)
+    alive = st2["status"] == 0
+    assert torch.all(st2["t"][alive] == 0.4e-5)
+    K.catapult_trace_continue(c["gf"], cfg["params"], st2)
+    assert torch.equal(st2["status"], g["status"])
+    d = (st2["x"] - g["xf"]).cpu().numpy()
+    d[1] = np.remainder(d[1] + math.pi, 2 * math.pi) - math.pi
+    assert np.all(np.abs(d) <= 1e-8 * np.array([1, 1, 10, W.V_TOTAL])[:, None])
+    K.catapult_trace_continue(c["gf"], cfg["params"], st2)   # nothing left to do: untouched
+    assert torch.equal(st2["status"], g["status"])
+
+
+def test_trace_host_equals_device(K, cases):
+    c = cases[4]
+    cfg = c["cfg"]
+    g = K.catapult_trace(c["gf"], cfg["params"], _dev(cfg["x0"]))
+    h = K.catapult_trace_host(c["gf"], cfg["params"], np.ascontiguousarray(cfg["x0"]))
+    assert np.array_equal(h["xf"], g["xf"].cpu().numpy())
+    assert np.array_equal(h["status"], g["status"].cpu().numpy())
+    assert np.array_equal(h["tstop"], g["tstop"].cpu().numpy())
+    assert h["counters"][0] == g["counters"][0].item()
+
+
+# ---- a10: estimate ---------------------------------------------------------------------------------
+def test_estimate_parity(K, oracle):
+    rng = np.random.default_rng(77)
+    for n in (1, 2, 31, 1000, 300_001):
+        status = rng.integers(0, 3, size=n).astype(np.int32)
+        tstop = rng.random(n) * 1e-3
+        for kind in (0, 1, 2):
+            got = K.catapult_estimate(kind, d_status=_dev(status), d_tstop=_dev(tstop), d_g_user=_dev(tstop ** 2))
+            want = oracle.estimate(kind, status=status, tstop=tstop, g_user=tstop ** 2)
+            if kind == 0:
+                assert got[2] == want[2] and got[0] == want[0]        # integer count: exact
+            assert np.allclose(got, want, rtol=1e-12, atol=1e-300)
+    with pytest.raises(K.CatapultError):
+        K.catapult_estimate(0, d_status=None, d_tstop=_dev(np.zeros(3)))

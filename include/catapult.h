@@ -147,6 +147,18 @@ catapult_status catapult_trace_continue_host(const catapult_field *f, const cata
                                              int64_t n, double *h_x, double *h_t, double *h_dt,
                                              double *h_mu, int32_t *h_status, uint32_t *h_nacc,
                                              uint32_t *h_nrej, uint64_t *h_counters);
+/* test hook: scripted replay.  Every particle starts at t = 0 from d_x0[4][n] and takes the step sizes
+   d_h[nsteps][n] (step-major) one after the other, each step ACCEPTED whatever its error ratio (the
+   controller is bypassed); a particle stops at its first h <= 0, after nsteps steps, or when an end
+   state is beyond the loss boundary.  d_r[nsteps][n] (may be NULL) receives Eq. 4's error ratio of every
+   step taken (other entries are left untouched).  d_xf, d_tstop, d_status as in catapult_trace
+   (status REACHED_T when the script ran out).  Adaptive runs in different arithmetic take different
+   accept/reject decisions and then differ by their global error; replaying one
+   run's accepted step sizes removes the decisions and leaves the step arithmetic to be compared. */
+catapult_status catapult_trace_scripted(const catapult_field *f, const catapult_trace_params *p, int64_t n,
+                                        const double *d_x0, int32_t nsteps, const double *d_h,
+                                        double *d_xf, double *d_tstop, int32_t *d_status, double *d_r,
+                                        void *stream);
 /* test hook: ONE attempted DP5 step of size d_h[i] from state d_x[4][n] at time d_t[n] (mu taken
    from the state as in catapult_trace_init): d_xnew[4][n], d_errratio[n] (Eq. 4),
    d_k[7][4][n] = the seven stage derivatives in the stepped variables */

@@ -495,6 +495,37 @@ int64_t orc_trace_record(const orc_field *f, const orc_params *p, const double x
   return nrec;
 }
 
+int64_t orc_trace_scripted(const orc_field *f, const orc_params *p, const double x0[4], int64_t nsteps,
+                           const double *h, double xf[4], double *tstop, int32_t *status, double *r) {
+  double y[4], k1[4], ynew[4], k7[4], err[4];
+  const double cscale[4] = {1.0, 1.0, 1.0, orc_vtotal(p)};
+  double t = 0.0;
+  int64_t taken = 0;
+  int32_t st = 0;
+  orc_state_to_y(f, x0, y);
+  if (orc_is_lost(f, y)) {
+    for (int i = 0; i < 4; ++i) xf[i] = x0[i];
+    *tstop = 0.0;
+    *status = 1;
+    return 0;
+  }
+  orc_rhs_ctx ctx = {f, p, orc_mu_init(f, p, x0)};
+  orc_rhs_cb(&ctx, t, y, k1);
+  while (taken < nsteps && h[taken] > 0.0) {
+    const double hh = h[taken];
+    orc_dp5_attempt(orc_rhs_cb, &ctx, 4, t, y, k1, hh, ynew, k7, err, NULL);
+    if (r) r[taken] = orc_error_ratio(4, err, y, k1, hh, p->rtol, p->atol, cscale);
+    ++taken;
+    t = t + hh;
+    for (int i = 0; i < 4; ++i) { y[i] = ynew[i]; k1[i] = k7[i]; }
+    if (orc_is_lost(f, y)) { st = 1; break; }
+  }
+  orc_y_to_state(f, y, xf);
+  *tstop = t;
+  *status = st;
+  return taken;
+}
+
 void orc_step_once(const orc_field *f, const orc_params *p, const double x[4], double t, double h,
                    double xnew[4], double *errratio, double *k) {
   double y[4], k1[4], ynew[4], k7[4], err[4];

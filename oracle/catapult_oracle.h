@@ -138,6 +138,14 @@ void orc_step_once(const orc_field *f, const orc_params *p, const double x[4], d
 int64_t orc_trace_record(const orc_field *f, const orc_params *p, const double x0[4], double *traj,
                          int64_t maxrec, double *tstop, int32_t *status);
 
+/* scripted replay of one particle (twin of catapult_trace_scripted): takes the step sizes h[0..nsteps)
+   one after the other from t=0, every step accepted whatever its error ratio (written to r[i]); stops
+   at the first h <= 0, after nsteps steps, or when an end state is beyond the loss boundary.  Returns
+   the number of steps taken; status 1 if lost else 0.  Lets a test walk another run's accepted-step
+   sequence without any accept/reject decision in between. */
+int64_t orc_trace_scripted(const orc_field *f, const orc_params *p, const double x0[4], int64_t nsteps,
+                           const double *h, double xf[4], double *tstop, int32_t *status, double *r);
+
 /* ---- estimator (Eq. 2) ---- */
 /* g_kind 0: 1[status==1], 1: tstop, 2: user array.  out = {mean, standard error, sum} */
 void orc_estimate(int g_kind, int64_t n, const int32_t *status, const double *tstop,

@@ -54,6 +54,7 @@ def lib():
         L.orc_error_ratio.restype = C.c_double
         L.orc_controller.restype = C.c_double
         L.orc_trace_record.restype = C.c_int64
+        L.orc_trace_scripted.restype = C.c_int64
         L.orc_max_threads.restype = C.c_int
     return _lib
 
@@ -267,6 +268,18 @@ def trace_record(f: Field, p: CParams, x0, maxrec: int = 200000):
     n = lib().orc_trace_record(f.ref, C.byref(p), _dp(x0), _dp(traj), C.c_int64(maxrec),
                                C.byref(ts), C.byref(st))
     return traj[:n].copy(), ts.value, st.value
+
+
+def trace_scripted(f: Field, p: CParams, x0, h):
+    """Replays the step sizes h (1-D) from x0; returns xf, tstop, status, r[steps taken]."""
+    x0, h = _f64(x0), _f64(h)
+    xf = np.zeros(4)
+    r = np.full(h.size, np.nan)
+    ts = C.c_double(0)
+    st = C.c_int32(0)
+    n = lib().orc_trace_scripted(f.ref, C.byref(p), _dp(x0), C.c_int64(h.size), _dp(h), _dp(xf),
+                                 C.byref(ts), C.byref(st), _dp(r))
+    return xf, ts.value, st.value, r[:n].copy()
 
 
 def estimate(g_kind, status=None, tstop=None, g_user=None):

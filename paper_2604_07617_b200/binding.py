@@ -24,7 +24,7 @@ EXPORTS = [
     "catapult_field_build", "catapult_field_build_host", "catapult_field_destroy",
     "catapult_field_table_bytes", "catapult_field_eval", "catapult_field_export_rows",
     "catapult_trace", "catapult_trace_init", "catapult_trace_continue", "catapult_trace_host",
-    "catapult_trace_continue_host",
+    "catapult_trace_continue_host", "catapult_trace_scripted",
     "catapult_step_once", "catapult_estimate", "catapult_measure_fp64_peak",
     "catapult_measure_l2_bandwidth", "catapult_trace_launch_shape", "catapult_last_error",
     "catapult_version",
@@ -78,6 +78,7 @@ def load():
     L.catapult_trace_continue.argtypes = [vp, C.POINTER(TraceParams), i64, dp, dp, dp, dp, dp, dp, dp, dp, vp]
     L.catapult_trace_host.argtypes = [vp, C.POINTER(TraceParams), i64, dp, dp, dp, dp, dp, dp, dp]
     L.catapult_trace_continue_host.argtypes = [vp, C.POINTER(TraceParams), i64, dp, dp, dp, dp, dp, dp, dp, dp]
+    L.catapult_trace_scripted.argtypes = [vp, C.POINTER(TraceParams), i64, dp, C.c_int32, dp, dp, dp, dp, dp, vp]
     L.catapult_step_once.argtypes = [vp, C.POINTER(TraceParams), i64, dp, dp, dp, dp, dp, dp, vp]
     L.catapult_estimate.argtypes = [C.c_int32, i64, dp, dp, dp, dp, dp, vp]
     L.catapult_measure_fp64_peak.argtypes = [C.POINTER(C.c_double)]
@@ -292,6 +293,23 @@ def catapult_trace_continue_host(f: Field, pd: dict, st: dict) -> dict:
         _hptr(st["mu"], np.float64), _hptr(st["status"], np.int32), _hptr(st.get("nacc"), np.uint32),
         _hptr(st.get("nrej"), np.uint32), _hptr(st.get("counters"), np.uint64)))
     return st
+
+
+def catapult_trace_scripted(f: Field, pd: dict, d_x0, d_h) -> dict:
+    """Replays the step sizes d_h [nsteps][n] (CUDA float64) from d_x0 [4][n]; every step is accepted."""
+    torch = _torch()
+    p = make_params(pd)
+    n = d_x0.shape[1]
+    nsteps = d_h.shape[0]
+    dev = d_x0.device
+    xf = torch.empty((4, n), dtype=torch.float64, device=dev)
+    tstop = torch.empty(n, dtype=torch.float64, device=dev)
+    status = torch.empty(n, dtype=torch.int32, device=dev)
+    r = torch.full((nsteps, n), float("nan"), dtype=torch.float64, device=dev)
+    _check(load().catapult_trace_scripted(f._h, C.byref(p), n, _ptr(d_x0, torch.float64), nsteps,
+                                          _ptr(d_h, torch.float64), _ptr(xf), _ptr(tstop), _ptr(status), _ptr(r),
+                                          _stream()))
+    return dict(xf=xf, tstop=tstop, status=status, r=r)
 
 
 def catapult_step_once(f: Field, pd: dict, d_x, d_t, d_h):

@@ -229,7 +229,7 @@ catapult_status catapult_field_export_rows(const catapult_field* f, double* d_ou
 }
 
 static catapult_status run_trace(const catapult_field* f, const catapult_trace_params* p, TraceArgs a,
-                                 cudaStream_t s) {
+                                 cudaStream_t s, bool scripted = false) {
   TraceConst tc;
   int model = 0;
   catapult_status st = make_trace_const(f, p, &tc, &model);
@@ -245,7 +245,7 @@ static catapult_status run_trace(const catapult_field* f, const catapult_trace_p
     return cuda_fail(e, "cudaMemsetAsync(queue)");
   }
   a.queue = queue;
-  st = launch_trace(tc, a, model, s);
+  st = scripted ? launch_trace_scripted(tc, a, model, s) : launch_trace(tc, a, model, s);
   cudaFreeAsync(queue, s);
   return st;
 }
@@ -266,6 +266,24 @@ catapult_status catapult_trace(const catapult_field* f, const catapult_trace_par
   a.nrej = d_nrej;
   a.counters = (unsigned long long*)d_counters;
   return run_trace(f, p, a, (cudaStream_t)stream);
+}
+
+catapult_status catapult_trace_scripted(const catapult_field* f, const catapult_trace_params* p, int64_t n,
+                                        const double* d_x0, int32_t nsteps, const double* d_h, double* d_xf,
+                                        double* d_tstop, int32_t* d_status, double* d_r, void* stream) {
+  if (n < 0 || nsteps < 0) return fail(CATAPULT_EINVAL, "n < 0 or nsteps < 0");
+  if (n > 0 && (!d_x0 || !d_xf || !d_tstop || !d_status || (nsteps > 0 && !d_h)))
+    return fail(CATAPULT_EINVAL, "d_x0, d_h, d_xf, d_tstop and d_status are required");
+  TraceArgs a{};
+  a.n = n;
+  a.x_in = d_x0;
+  a.x_out = d_xf;
+  a.t_io = d_tstop;
+  a.status = d_status;
+  a.script_h = d_h;
+  a.script_r = d_r;
+  a.script_len = nsteps;
+  return run_trace(f, p, a, (cudaStream_t)stream, true);
 }
 
 catapult_status catapult_trace_init(const catapult_field* f, const catapult_trace_params* p, int64_t n,

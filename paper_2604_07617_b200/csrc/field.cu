@@ -27,16 +27,26 @@ field_build_kernel(const double* __restrict__ nodes, double* __restrict__ table,
   }
 }
 
-template <int NQ, bool DIM1_PERIODIC>
-__global__ void field_eval_kernel(const __grid_constant__ FieldConst f, long long npts, const double* __restrict__ pts,
-                                  double* __restrict__ out) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= npts) return;
-  double u[3], fv[NQ];
-  const long long cell = locate<DIM1_PERIODIC>(f, pts[i], pts[npts + i], pts[2 * npts + i], u);
-  tricubic_cell<NQ>(f.table + cell * (NQ * 64), u, fv);
+// test hook: the production evaluation path (group of NL lanes per point, coefficients staged through
+// the on-chip cell cache) at arbitrary points
+template <int MODEL>
+__global__ void __launch_bounds__(ModelTraits<MODEL>::NT, ModelTraits<MODEL>::MINB)
+field_eval_kernel(const __grid_constant__ FieldConst f, long long npts, const double* __restrict__ pts,
+                  double* __restrict__ out) {
+  using MT = ModelTraits<MODEL>;
+  extern __shared__ double2 smem[];
+  const Group<MT::NL> g;
+  CellCache<MODEL> cc;
+  cc.init(smem);
+  const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) / MT::NL;
+  if (i >= npts) return;  // group-uniform
+  double u[3], fv[MT::NQ];
+  const long long cell = locate<!MT::CART>(f, pts[i], pts[npts + i], pts[2 * npts + i], u);
+  tricubic_group<MODEL>(f, g, cc, cell, u, fv);
+  if (g.j == 0) {
 #pragma unroll
-  for (int q = 0; q < NQ; ++q) out[(long long)q * npts + i] = fv[q];
+    for (int q = 0; q < MT::NQ; ++q) out[(long long)q * npts + i] = fv[q];
+  }
 }
 
 // table [cell][q][64] -> rows [(cell*64+node)][q]  (row = node, column = quantity)
@@ -68,17 +78,24 @@ catapult_status launch_field_build(const catapult_field_desc& d, const double* d
   return CATAPULT_OK;
 }
 
+template <int MODEL>
+static catapult_status field_eval_one(const FieldConst& fc, int64_t npts, const double* d_pts, double* d_out,
+                                      cudaStream_t s) {
+  using MT = ModelTraits<MODEL>;
+  CATAPULT_CUDA_TRY(cudaFuncSetAttribute(field_eval_kernel<MODEL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)MT::SMEM_BYTES));
+  const long long per_block = MT::NT / MT::NL;
+  const int blocks = (int)((npts + per_block - 1) / per_block);
+  field_eval_kernel<MODEL><<<blocks, MT::NT, MT::SMEM_BYTES, s>>>(fc, npts, d_pts, d_out);
+  CATAPULT_CUDA_TRY(cudaGetLastError());
+  return CATAPULT_OK;
+}
+
 catapult_status launch_field_eval(const FieldConst& fc, int64_t npts, const double* d_pts, double* d_out,
                                   cudaStream_t s) {
   if (npts == 0) return CATAPULT_OK;
-  const int threads = 128;
-  const int blocks = (int)((npts + threads - 1) / threads);
-  if (fc.coord == CATAPULT_COORD_BOOZER)
-    field_eval_kernel<CATAPULT_NQUANT_BOOZER, true><<<blocks, threads, 0, s>>>(fc, npts, d_pts, d_out);
-  else
-    field_eval_kernel<CATAPULT_NQUANT_CYL, false><<<blocks, threads, 0, s>>>(fc, npts, d_pts, d_out);
-  CATAPULT_CUDA_TRY(cudaGetLastError());
-  return CATAPULT_OK;
+  if (fc.coord == CATAPULT_COORD_BOOZER) return field_eval_one<MODEL_BOOZER_VAC>(fc, npts, d_pts, d_out, s);
+  return field_eval_one<MODEL_CART>(fc, npts, d_pts, d_out, s);
 }
 
 catapult_status launch_field_export_rows(const FieldConst& fc, int64_t ncells, double* d_out, cudaStream_t s) {

@@ -45,6 +45,10 @@ struct TraceArgs {
   unsigned long long* queue;     // work counter, zero at launch
   int resume;     // 1: continue from (t,dt,mu,status) arrays
   int init_only;  // 1: only fill (t,dt,mu,status)
+  // scripted replay (catapult_trace_scripted): step sizes are read instead of controlled
+  const double* script_h;  // [script_len][n]; a particle stops at the first h <= 0
+  double* script_r;        // [script_len][n] error ratio of every scripted step (nullable)
+  int script_len;
 };
 
 void set_error(const std::string& msg);
@@ -65,6 +69,7 @@ catapult_status launch_field_export_rows(const FieldConst& fc, int64_t ncells, d
 
 // tracer.cu
 catapult_status launch_trace(const TraceConst& tc, const TraceArgs& a, int model, cudaStream_t s);
+catapult_status launch_trace_scripted(const TraceConst& tc, const TraceArgs& a, int model, cudaStream_t s);
 catapult_status launch_step_once(const TraceConst& tc, int model, int64_t n, const double* d_x, const double* d_t,
                                  const double* d_h, double* d_xnew, double* d_err, double* d_k, cudaStream_t s);
 catapult_status trace_launch_shape(int model, int64_t n, int* blocks, int* threads);

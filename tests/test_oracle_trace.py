@@ -140,3 +140,45 @@ def test_estimator_matches_numpy(oracle):
     assert abs(out[0] - tstop.mean()) < 1e-14 and abs(out[1] - tstop.std(ddof=0) / math.sqrt(999)) < 1e-12
     out = O.estimate(2, status=status, tstop=tstop, g_user=tstop ** 2)
     assert abs(out[0] - (tstop ** 2).mean()) < 1e-14
+
+
+def test_scripted_replay_reproduces_the_adaptive_trace(oracle):
+    """orc_trace_scripted walks a given accepted-step sequence with no accept/reject decision.  Pins:
+    (i) fed the step sizes the adaptive trace accepted, it lands on the adaptive trace's end state (the
+    sizes are differences of recorded times, equal to the attempted h up to one rounding of t);
+    (ii) the error ratios it reports are all <= 1 (they were accepted) and equal one-step ratios
+    computed independently through step_once from the recorded states;
+    (iii) a script of one step equals step_once; an empty script returns the initial state."""
+    O = oracle
+    for idx, kw in ((0, dict(n=3, T=1e-5)), (3, dict(n=2, T=1e-5, ncell=[12, 11, 5])),
+                    (4, dict(n=2, T=1e-5, ncell=[12, 10, 9]))):
+        cfg = W.config(idx, **kw)
+        f, p = O.Field(cfg["field"]), O.make_params(cfg["params"])
+        full = O.trace(f, p, cfg["x0"])
+        for i in range(cfg["x0"].shape[1]):
+            x0 = cfg["x0"][:, i]
+            traj, ts, st = O.trace_record(f, p, x0)
+            h = np.diff(traj[:, 0])
+            assert len(h) == full["nacc"][i]
+            xf, t_end, st2, r = O.trace_scripted(f, p, x0, h)
+            assert st2 == st == full["status"][i] and len(r) == len(h)
+            assert abs(t_end - ts) <= 1e-15 * ts * len(h)
+            d = xf - full["xf"][:, i]
+            d[1] = math.remainder(d[1], 2 * math.pi)
+            sc = np.maximum(np.abs(full["xf"][:, i]), [1.0, 1.0, 1.0, W.V_TOTAL])
+            assert np.all(np.abs(d) <= 1e-12 * sc * len(h)), d
+            assert np.all(r <= 1.0 + 1e-3)
+            for j in (0, len(h) // 2, len(h) - 2):
+                # traj row = (t, state in the API's coordinates).  r is a quotient of a difference that
+                # cancels to ~1e-9 of its terms: a few per cent of round-off noise is its own precision
+                # (DESIGN.md "Tolerances"); the clamped last step can be arbitrarily short and is left out
+                _, rj, _ = O.step_once(f, p, traj[j, 1:5], traj[j, 0], h[j])
+                assert abs(rj - r[j]) <= 5e-2 * max(r[j], 1e-3), (j, rj, r[j])
+            x1, t1, s1, r1 = O.trace_scripted(f, p, x0, h[:1])
+            xs, rs, _ = O.step_once(f, p, x0, 0.0, h[0])
+            assert np.array_equal(x1, xs) and r1[0] == rs and t1 == h[0]
+            xe, te, se, re = O.trace_scripted(f, p, x0, np.zeros(0))
+            de = xe - x0
+            if idx != 3:
+                de[1] = math.remainder(de[1], 2 * math.pi)   # theta is returned in (-pi, pi]
+            assert te == 0.0 and len(re) == 0 and np.all(np.abs(de) <= 1e-15 * np.maximum(1.0, np.abs(x0)))

@@ -187,6 +187,21 @@ catapult_status catapult_measure_l2_bandwidth(size_t bytes, double *bytes_per_s)
 catapult_status catapult_trace_launch_shape(const catapult_field *f, const catapult_trace_params *p,
                                             int32_t *blocks, int32_t *threads);
 
+/* test hook: the device-side fp64 elementary functions the tracer's scalar path uses (csrc/gc_math.cuh)
+   evaluated elementwise on d_a[n] (and d_b[n] where a second argument exists):
+     ATAN2: out0 = atan2(a, b);  SINCOS: out0 = sin(a), out1 = cos(a);  EXP: out0 = exp(a);
+     SQRT_RSQRT: out0 = sqrt(a), out1 = 1/sqrt(a);  RCP: out0 = 1/a;
+     POW_NEG_INV: out0 = a^(-1/5), out1 = a^(-1/3) (the step-size controller's powers).
+   d_b and d_out1 may be NULL where unused. */
+#define CATAPULT_FN_ATAN2 0
+#define CATAPULT_FN_SINCOS 1
+#define CATAPULT_FN_EXP 2
+#define CATAPULT_FN_SQRT_RSQRT 3
+#define CATAPULT_FN_RCP 4
+#define CATAPULT_FN_POW_NEG_INV 5
+catapult_status catapult_math_probe(int32_t fn, int64_t n, const double *d_a, const double *d_b,
+                                    double *d_out0, double *d_out1, void *stream);
+
 const char *catapult_last_error(void);
 const char *catapult_version(void);
 

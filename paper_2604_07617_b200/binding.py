@@ -25,7 +25,7 @@ EXPORTS = [
     "catapult_field_table_bytes", "catapult_field_eval", "catapult_field_export_rows",
     "catapult_trace", "catapult_trace_init", "catapult_trace_continue", "catapult_trace_host",
     "catapult_trace_continue_host", "catapult_trace_scripted",
-    "catapult_step_once", "catapult_estimate", "catapult_measure_fp64_peak",
+    "catapult_step_once", "catapult_estimate", "catapult_math_probe", "catapult_measure_fp64_peak",
     "catapult_measure_l2_bandwidth", "catapult_trace_launch_shape", "catapult_last_error",
     "catapult_version",
 ]
@@ -81,6 +81,7 @@ def load():
     L.catapult_trace_scripted.argtypes = [vp, C.POINTER(TraceParams), i64, dp, C.c_int32, dp, dp, dp, dp, dp, vp]
     L.catapult_step_once.argtypes = [vp, C.POINTER(TraceParams), i64, dp, dp, dp, dp, dp, dp, vp]
     L.catapult_estimate.argtypes = [C.c_int32, i64, dp, dp, dp, dp, dp, vp]
+    L.catapult_math_probe.argtypes = [C.c_int32, i64, dp, dp, dp, dp, vp]
     L.catapult_measure_fp64_peak.argtypes = [C.POINTER(C.c_double)]
     L.catapult_measure_l2_bandwidth.argtypes = [C.c_size_t, C.POINTER(C.c_double)]
     L.catapult_trace_launch_shape.argtypes = [vp, C.POINTER(TraceParams), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
@@ -335,6 +336,18 @@ def catapult_estimate(g_kind: int, d_status=None, d_tstop=None, d_g_user=None, t
     _check(load().catapult_estimate(g_kind, n, _ptr(d_status, torch.int32, True), _ptr(d_tstop, torch.float64, True),
                                     _ptr(d_g_user, torch.float64, True), _ptr(out), _hptr(h, np.float64), _stream()))
     return h if to_host else out
+
+
+FN_ATAN2, FN_SINCOS, FN_EXP, FN_SQRT_RSQRT, FN_RCP, FN_POW_NEG_INV = range(6)
+
+
+def catapult_math_probe(fn: int, d_a, d_b=None):
+    """Test hook: (out0, out1) of the device-side elementary function `fn` on CUDA float64 tensors."""
+    torch = _torch()
+    o0, o1 = torch.empty_like(d_a), torch.empty_like(d_a)
+    _check(load().catapult_math_probe(fn, d_a.numel(), _ptr(d_a, torch.float64), _ptr(d_b, torch.float64, True),
+                                      _ptr(o0), _ptr(o1), _stream()))
+    return o0, o1
 
 
 def catapult_measure_fp64_peak() -> float:

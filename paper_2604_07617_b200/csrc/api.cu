@@ -92,6 +92,7 @@ static catapult_status make_trace_const(const catapult_field* f, const catapult_
   }
   tc->f = f->fc;
   tc->M = p->mass;
+  tc->invM = 1.0 / p->mass;
   tc->q = p->charge;
   tc->Moq = p->mass / p->charge;
   tc->vtot = std::sqrt(2.0 * p->energy / p->mass);
@@ -125,6 +126,7 @@ static catapult_status make_trace_const(const catapult_field* f, const catapult_
   tc->saw_s0 = p->saw_s0;
   tc->saw_invw2 = p->saw_on ? 1.0 / p->saw_w2 : 0.0;
   tc->saw_omega = p->saw_omega;
+  tc->saw_inv_omG = p->saw_on ? f->fc.invG / p->saw_omega : 0.0;
   *model = f->desc.coord == CATAPULT_COORD_CYL ? MODEL_CART : (p->saw_on ? MODEL_BOOZER_SAW : MODEL_BOOZER_VAC);
   (void)E_CHARGE;
   return CATAPULT_OK;
@@ -454,6 +456,15 @@ catapult_status catapult_estimate(int32_t g_kind, int64_t n, const int32_t* d_st
     CATAPULT_CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
   }
   return CATAPULT_OK;
+}
+
+catapult_status catapult_math_probe(int32_t fn, int64_t n, const double* d_a, const double* d_b, double* d_out0,
+                                    double* d_out1, void* stream) {
+  if (n < 0) return fail(CATAPULT_EINVAL, "n < 0");
+  if (fn < 0 || fn > CATAPULT_FN_POW_NEG_INV) return fail(CATAPULT_EINVAL, "unknown fn");
+  if (n > 0 && (!d_a || !d_out0)) return fail(CATAPULT_EINVAL, "d_a/d_out0 is NULL");
+  if (n > 0 && fn == CATAPULT_FN_ATAN2 && !d_b) return fail(CATAPULT_EINVAL, "atan2 needs d_b");
+  return launch_math_probe(fn, n, d_a, d_b, d_out0, d_out1, (cudaStream_t)stream);
 }
 
 catapult_status catapult_measure_fp64_peak(double* flops_per_s) {

@@ -14,6 +14,7 @@
 #pragma once
 
 #include "internal.h"
+#include "gc_math.cuh"
 
 namespace catapult {
 
@@ -132,21 +133,21 @@ __device__ __forceinline__ void lagrange4(double u, double L[4]) {
   L[3] = 4.5 * p01 * t2;
 }
 
-// reduces x-lo into [0, span) (periodic dimension)
+// reduces x-lo into [0, span) (periodic dimension).  span * floor(.) is exact inside the fma, so the result
+// carries one rounding; a result that lands a rounding outside [0, span) is handled by the cell clamp
+// (u marginally outside [0,1] on a face, where the two cells agree: DESIGN.md Q8, Q9).
 __device__ __forceinline__ double wrap_periodic(double xr, double span, double invspan) {
-  double r = fma(-span, floor(xr * invspan), xr);
-  if (r < 0.0) r += span;
-  if (r >= span) r -= span;
-  if (!(r >= 0.0 && r < span)) r = 0.0;
-  return r;
+  return fma(-span, floor(xr * invspan), xr);
 }
 
+// cell index clamped to [0, k-1] and local coordinate u = t - cell (outside [0,1] => extrapolation).
+// The floor is taken by the fp64 -> int32 conversion (saturating; NaN -> 0) and clamped in integers.
 __device__ __forceinline__ int cell_and_u(double xr, double invh, int k, double& u) {
   const double t = xr * invh;
-  double fi = floor(t);
-  fi = fmin(fmax(fi, 0.0), (double)(k - 1));
-  u = t - fi;
-  return (int)fi;
+  int i = __double2int_rd(t);
+  i = min(max(i, 0), k - 1);
+  u = t - (double)i;
+  return i;
 }
 
 // x = grid coordinates (dim 0 never periodic; dim 1 periodic for Boozer; dim 2 always periodic)
@@ -287,18 +288,18 @@ __device__ __forceinline__ void rhs(const TraceConst& tc, const Group<ModelTrait
   double fv[NQ], u[3];
   if (MODEL == MODEL_CART) {
     const double R2 = fma(y[0], y[0], y[1] * y[1]);
-    const double R = sqrt(R2);
-    const double phi = atan2(y[1], y[0]);
+    double R, invR;
+    fm::sqrt_rsqrt(R2, R, invR);
+    const double phi = fm::atan2(y[1], y[0]);
     const long long cell = locate<false>(f, R, y[2], phi, u);
     tricubic_group<MODEL>(f, g, cc, cell, u, fv);
-    const double invR = 1.0 / R;
     const double cph = y[0] * invR, sph = y[1] * invR;
     const double BR = fv[0], Bp = fv[1], BZ = fv[2], gR = fv[3], gp = fv[4], gZ = fv[5];
     const double Bx = BR * cph - Bp * sph, By = BR * sph + Bp * cph, Bz = BZ;
     const double gx = gR * cph - gp * sph, gy = gR * sph + gp * cph, gz = gZ;
     const double B2 = fma(BR, BR, fma(Bp, Bp, BZ * BZ));
-    const double B = sqrt(B2);
-    const double invB = 1.0 / B;
+    double B, invB;
+    fm::sqrt_rsqrt(B2, B, invB);
     const double vpar = y[3];
     // (M/(q|B|^3)) (vperp^2/2 + vpar^2),  vperp^2 = 2 mu |B|
     const double coef = tc.Moq * invB * invB * invB * fma(mu, B, vpar * vpar);
@@ -312,13 +313,14 @@ __device__ __forceinline__ void rhs(const TraceConst& tc, const Group<ModelTrait
     level = fv[6];
   } else {
     const double s2 = fma(y[0], y[0], y[1] * y[1]);
-    const double s = sqrt(s2);
-    const double theta = atan2(y[1], y[0]);
+    double s, invs;
+    fm::sqrt_rsqrt(s2, s, invs);
+    const double theta = fm::atan2(y[1], y[0]);
     const long long cell = locate<true>(f, s, theta, y[2], u);
     tricubic_group<MODEL>(f, g, cc, cell, u, fv);
     const double B = fv[0], B_s = fv[1], B_th = fv[2], B_ze = fv[3];
     const double vpar = y[3];
-    const double invB = 1.0 / B;
+    const double invB = fm::rcp(B);
     const double W = tc.Moq * fma(vpar * vpar, invB, mu);
     const double iota = fma(f.iota1, s, f.iota0);
     const double B_psi = B_s * f.invpsi0;
@@ -332,17 +334,17 @@ __device__ __forceinline__ void rhs(const TraceConst& tc, const Group<ModelTrait
       // Phi = Phihat(s) sin(m th - n ze + w t); alpha = -(iota m - n) Phi / (w G)  (E_par = 0)
       const double mm = (double)tc.saw_m, nn = (double)tc.saw_n, om = tc.saw_omega;
       const double ds = s - tc.saw_s0;
-      const double Phihat = tc.saw_Phi0 * exp(-ds * ds * tc.saw_invw2);
+      const double Phihat = tc.saw_Phi0 * fm::exp(-ds * ds * tc.saw_invw2);
       const double dPhihat = Phihat * (-2.0 * ds * tc.saw_invw2);
       const double eta = fma(mm, theta, fma(-nn, y[2], om * t));
       double sn, cs;
-      sincos(eta, &sn, &cs);
+      fm::sincos(eta, sn, cs);
       const double Phi = Phihat * sn;
       const double Phi_psi = dPhihat * sn * f.invpsi0;
       const double Phi_th = mm * Phihat * cs;
       const double Phi_ze = -nn * Phihat * cs;
       const double kpar = fma(iota, mm, -nn);
-      const double inv_omG = f.invG / om;
+      const double inv_omG = tc.saw_inv_omG;
       const double al_th = -kpar * Phi_th * inv_omG;
       const double al_t = -kpar * Phihat * cs * f.invG;
       const double al_psi = -fma(f.iota1 * mm, Phi, kpar * dPhihat * sn) * inv_omG * f.invpsi0;
@@ -352,9 +354,8 @@ __device__ __forceinline__ void rhs(const TraceConst& tc, const Group<ModelTrait
       thdot = fma(B_psi, W, fma(iag * f.invG, vpar * B, Phi_psi));
       const double t1 = tc.M * mu * fma(al_th * B_psi, f.G, fma(B_th, iag, B_ze));
       const double t2 = tc.q * fma(al_t, f.G, fma(al_th * f.G, Phi_psi, fma(iag, Phi_th, Phi_ze)));
-      vdot = fma(-(B * f.invG / tc.M), t1 + t2, vpar * invB * fma(B_th, Phi_psi, -B_psi * Phi_th));
+      vdot = fma(-(B * f.invG * tc.invM), t1 + t2, vpar * invB * fma(B_th, Phi_psi, -B_psi * Phi_th));
     }
-    const double invs = (s > 0.0) ? 1.0 / s : 0.0;
     const double c = (s > 0.0) ? y[0] * invs : 1.0;
     const double sn_ = y[1] * invs;
     dy[0] = fma(sdot, c, -thdot * y[1]);
@@ -470,7 +471,7 @@ __device__ __forceinline__ double error_ratio(const TraceConst& tc, const Group<
     const bool is_v = (i * NL + g.j == 3);
     const double sc = is_v ? tc.atol * tc.vtot : tc.atol;
     const double den = fma(tc.rtol, fma(ah, fabs(k1m[i]), fabs(pick<NL>(y, i, g.j))), sc);
-    const double v = fabs(errm[i]) / den;
+    const double v = fabs(errm[i]) * fm::rcp(den);
     chk += v;
     r = fmax(r, v);
   }
@@ -481,15 +482,14 @@ __device__ __forceinline__ double error_ratio(const TraceConst& tc, const Group<
 
 // Boost odeint default step adjuster for dopri5 (S2):
 //   r > 1  : reject, dt <- dt max(0.9 r^(-1/3), 1/5);  r < 0.5: accept, dt <- dt 0.9 max(r, 5^-5)^(-1/5).
-// Both powers are taken as exp(e log(x)) on one code path (relative error ~1e-15, far below the
+// Both powers are taken by fm::pow_neg_inv on one code path (relative error ~1e-15, far below the
 // sensitivity of anything downstream) so that lanes that grow and lanes that shrink do not diverge.
 __device__ __forceinline__ double controller(double h, double r, double dtmax, bool& accepted) {
   accepted = (r <= 1.0);
   double dt = h;
   if (!accepted || r < 0.5) {
-    const double ex = accepted ? -0.2 : (-1.0 / 3.0);
     const double base = accepted ? fmax(r, 1.0 / 3125.0) : r;
-    double fac = 0.9 * exp(ex * log(base));
+    double fac = 0.9 * fm::pow_neg_inv(base, accepted);
     if (!accepted && !(fac >= 0.2)) fac = 0.2;
     dt = h * fac;
   }

@@ -23,12 +23,12 @@ struct FieldConst {
 
 struct TraceConst {
   FieldConst f;
-  double M, q, Moq, vtot, vtot2;
+  double M, invM, q, Moq, vtot, vtot2;
   double T, rtol, atol, dt0, dtmax;
   long long max_steps;
   int max_rej;
   int saw_m, saw_n;
-  double saw_Phi0, saw_s0, saw_invw2, saw_omega;
+  double saw_Phi0, saw_s0, saw_invw2, saw_omega, saw_inv_omG;
 };
 
 struct TraceArgs {
@@ -77,6 +77,10 @@ catapult_status trace_launch_shape(int model, int64_t n, int* blocks, int* threa
 // estimate.cu
 catapult_status launch_estimate(int g_kind, int64_t n, const int* d_status, const double* d_tstop,
                                 const double* d_g, double* d_out, cudaStream_t s);
+
+// mathprobe.cu
+catapult_status launch_math_probe(int fn, int64_t n, const double* d_a, const double* d_b, double* d_o0, double* d_o1,
+                                  cudaStream_t s);
 
 // peaks.cu
 catapult_status measure_fp64_peak(double* flops);

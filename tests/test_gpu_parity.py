@@ -198,7 +198,7 @@ def test_trajectory_parity_1e5_window(K, oracle, cases, idx):
 @pytest.mark.parametrize("idx", [0, 1, 2, 3, 4])
 def test_adaptive_trace_1e5_window(K, oracle, cases, idx):
     """The free-running adaptive kernel against the adaptive oracle: statuses, stop times, counters, and
-    end states within the method's own global error bound (_free_diff_over_tol)."""
+    end states within the method's own global error (_free_diff_over_tol) of a converged orbit."""
     c = cases[idx]
     cfg = c["cfg"]
     g = K.catapult_trace(c["gf"], cfg["params"], _dev(cfg["x0"]))
@@ -206,9 +206,16 @@ def test_adaptive_trace_1e5_window(K, oracle, cases, idx):
     gs = g["status"].cpu().numpy()
     assert np.array_equal(gs, o["status"])
     gx, gt = g["xf"].cpu().numpy(), g["tstop"].cpu().numpy()
-    q = _free_diff_over_tol(cfg["field"]["coord"], gx, o["xf"], o["nacc"].astype(float), cfg["params"]["rtol"])
+    # both adaptive runs against a converged orbit (the oracle at rtol = 1e-12): each sits within the method's
+    # global error of it, and the GPU run is no further from it than the oracle's own run is (x3)
+    ref = oracle.trace(c["of"], oracle.make_params(dict(cfg["params"], rtol=1e-12, atol=1e-15)), cfg["x0"])
+    assert np.array_equal(ref["status"], gs)
+    nacc, rtol, coord = o["nacc"].astype(float), cfg["params"]["rtol"], cfg["field"]["coord"]
+    qg = _free_diff_over_tol(coord, gx, ref["xf"], nacc, rtol)
+    qo = _free_diff_over_tol(coord, o["xf"], ref["xf"], nacc, rtol)
     alive = gs == 0
-    assert np.all(q[:, alive] <= 1.0), q.max(axis=1)
+    for comp in range(4):
+        assert qg[comp, alive].max() <= max(1.0, 3.0 * qo[comp, alive].max()), (comp, qg[comp].max(), qo[comp].max())
     assert np.all(gt[alive] == cfg["params"]["T"])
     assert np.allclose(gt[~alive], o["tstop"][~alive], rtol=0.05)
     # step counts are integers decided by floating point: close, not identical
@@ -346,8 +353,8 @@ def test_refill_queue_many_more_particles_than_threads(K, oracle):
     x0 = np.tile(b_cfg["x0"], (1, reps))
     n = x0.shape[1]
     assert n > 2 * blocks * threads
-    x0[0, ::7] = 1.5                       # born outside: finish at once
     x0[0, 1::5] = 0.995                    # near the edge: many are lost early
+    x0[0, ::7] = 1.5                       # born outside: finish at once
     g = K.catapult_trace(gf, b_cfg["params"], _dev(x0))
     gs, gx = g["status"].cpu().numpy(), g["xf"].cpu().numpy()
     assert np.all((gs == 0) | (gs == 1))
@@ -413,3 +420,49 @@ def test_estimate_parity(K, oracle):
             assert np.allclose(got, want, rtol=1e-12, atol=1e-300)
     with pytest.raises(K.CatapultError):
         K.catapult_estimate(0, d_status=None, d_tstop=_dev(np.zeros(3)))
+
+
+def test_device_math_parity(K):
+    """The device-side elementary functions of csrc/gc_math.cuh (catapult_math_probe) against numpy on the
+    argument ranges the tracer produces: a few ulp.  (The oracle calls libm; the field, single-step and
+    trajectory parities above then bound what these differences do downstream.)"""
+    rng = np.random.default_rng(11)
+    n = 200_001
+    eps = np.finfo(float).eps
+
+    def rel(a, b):
+        return np.max(np.abs(a - b) / np.maximum(np.abs(b), 1e-300))
+
+    # atan2 over all octants and magnitudes (incl. axes and the origin)
+    y = rng.normal(size=n) * 10.0 ** rng.uniform(-6, 1, n)
+    x = rng.normal(size=n) * 10.0 ** rng.uniform(-6, 1, n)
+    y[:6] = [0.0, 0.0, 1.0, -1.0, 0.0, 1e-300]
+    x[:6] = [0.0, 1.0, 0.0, 0.0, -1.0, 1e-300]
+    g = K.catapult_math_probe(K.FN_ATAN2, _dev(y), _dev(x))[0].cpu().numpy()
+    e = np.arctan2(y, x)
+    assert np.max(np.abs(g - e)) <= 4 * eps * math.pi and rel(g[6:], e[6:]) <= 8 * eps
+    assert g[0] == 0.0 and g[4] == math.pi
+    # sincos: wave phases up to |eta| ~ 1e5 rad
+    a = rng.uniform(-1e5, 1e5, n)
+    a[:3] = [0.0, math.pi / 4, -math.pi / 2]
+    s, c = (t.cpu().numpy() for t in K.catapult_math_probe(K.FN_SINCOS, _dev(a)))
+    assert np.max(np.abs(s - np.sin(a))) <= 4 * eps and np.max(np.abs(c - np.cos(a))) <= 4 * eps
+    # exp of the wave envelope's exponent (<= 0) and a little beyond
+    a = np.concatenate([-rng.uniform(0, 700, n - 1000), rng.uniform(0, 5, 1000)])
+    g = K.catapult_math_probe(K.FN_EXP, _dev(a))[0].cpu().numpy()
+    assert rel(g, np.exp(a)) <= 4 * eps
+    # sqrt / rsqrt / rcp
+    a = 10.0 ** rng.uniform(-12, 12, n)
+    s, r = (t.cpu().numpy() for t in K.catapult_math_probe(K.FN_SQRT_RSQRT, _dev(a)))
+    assert rel(s, np.sqrt(a)) <= 2 * eps and rel(r, 1.0 / np.sqrt(a)) <= 3 * eps
+    z = K.catapult_math_probe(K.FN_SQRT_RSQRT, _dev(np.zeros(4)))
+    assert torch.all(z[0] == 0) and torch.all(z[1] == 0)
+    b = a * np.where(rng.random(n) < 0.5, -1.0, 1.0)
+    g = K.catapult_math_probe(K.FN_RCP, _dev(b))[0].cpu().numpy()
+    assert rel(g, 1.0 / b) <= 3 * eps
+    # controller powers: r in [5^-5, 1e30]
+    a = 10.0 ** rng.uniform(math.log10(1 / 3125), 30, n)
+    p5, p3 = (t.cpu().numpy() for t in K.catapult_math_probe(K.FN_POW_NEG_INV, _dev(a)))
+    assert rel(p5, a ** -0.2) <= 8 * eps and rel(p3, a ** (-1.0 / 3.0)) <= 8 * eps
+    bad = K.catapult_math_probe(K.FN_POW_NEG_INV, _dev(np.array([np.inf, np.nan, 1e300])))
+    assert not torch.any(bad[1] >= 0.2 / 0.9)       # the controller's floor takes over

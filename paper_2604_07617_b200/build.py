@@ -13,7 +13,7 @@ CSRC = os.path.join(PKG, "csrc")
 INC = os.path.join(ROOT, "include")
 LIB = os.path.join(PKG, "libcatapult.so")
 OBJ = os.path.join(PKG, "build")
-SOURCES = ["api.cu", "field.cu", "tracer.cu", "estimate.cu", "peaks.cu", "mathprobe.cu"]
+SOURCES = ["api.cu", "field.cu", "tracer.cu", "tracer_split.cu", "estimate.cu", "peaks.cu", "mathprobe.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-I", INC, "-I", CSRC]

@@ -2,6 +2,7 @@
 // parameter packing and stream-ordered launches.  No arithmetic of the method lives here.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -132,6 +133,12 @@ static catapult_status make_trace_const(const catapult_field* f, const catapult_
   return CATAPULT_OK;
 }
 
+// CATAPULT_TRACER=group selects the first-generation kernel (4-lane groups, tracer.cu) for A/B runs
+static bool use_group_tracer() {
+  const char* e = std::getenv("CATAPULT_TRACER");
+  return e && std::strcmp(e, "group") == 0;
+}
+
 static catapult_status use_device_of(const catapult_field* f) {
   int dev = -1;
   CATAPULT_CUDA_TRY(cudaGetDevice(&dev));
@@ -247,7 +254,8 @@ static catapult_status run_trace(const catapult_field* f, const catapult_trace_p
     return cuda_fail(e, "cudaMemsetAsync(queue)");
   }
   a.queue = queue;
-  st = scripted ? launch_trace_scripted(tc, a, model, s) : launch_trace(tc, a, model, s);
+  if (use_group_tracer()) st = scripted ? launch_trace_scripted(tc, a, model, s) : launch_trace(tc, a, model, s);
+  else st = launch_trace_split(tc, a, model, scripted ? 1 : 0, s);
   cudaFreeAsync(queue, s);
   return st;
 }
@@ -439,7 +447,29 @@ catapult_status catapult_step_once(const catapult_field* f, const catapult_trace
   if (st != CATAPULT_OK) return st;
   st = use_device_of(f);
   if (st != CATAPULT_OK) return st;
-  return launch_step_once(tc, model, n, d_x, d_t, d_h, d_xnew, d_errratio, d_k, (cudaStream_t)stream);
+  if (use_group_tracer())
+    return launch_step_once(tc, model, n, d_x, d_t, d_h, d_xnew, d_errratio, d_k, (cudaStream_t)stream);
+  if (n == 0) return CATAPULT_OK;
+  TraceArgs a{};
+  a.n = n;
+  a.x_in = d_x;
+  a.x_out = d_xnew;
+  a.t_io = const_cast<double*>(d_t);  // read only in this mode
+  a.script_h = d_h;
+  a.script_r = d_errratio;
+  a.kall = d_k;
+  cudaStream_t s = (cudaStream_t)stream;
+  unsigned long long* queue = nullptr;
+  CATAPULT_CUDA_TRY(cudaMallocAsync((void**)&queue, sizeof(unsigned long long), s));
+  cudaError_t e = cudaMemsetAsync(queue, 0, sizeof(unsigned long long), s);
+  if (e != cudaSuccess) {
+    cudaFreeAsync(queue, s);
+    return cuda_fail(e, "cudaMemsetAsync(queue)");
+  }
+  a.queue = queue;
+  st = launch_trace_split(tc, a, model, 2, s);
+  cudaFreeAsync(queue, s);
+  return st;
 }
 
 catapult_status catapult_estimate(int32_t g_kind, int64_t n, const int32_t* d_status, const double* d_tstop,
@@ -485,7 +515,8 @@ catapult_status catapult_trace_launch_shape(const catapult_field* f, const catap
   catapult_status st = make_trace_const(f, p, &tc, &model);
   if (st != CATAPULT_OK) return st;
   int b = 0, t = 0;
-  st = trace_launch_shape(model, (int64_t)1 << 40, &b, &t);
+  st = use_group_tracer() ? trace_launch_shape(model, (int64_t)1 << 40, &b, &t)
+                          : trace_split_launch_shape(model, (int64_t)1 << 40, &b, &t);
   *blocks = b;
   *threads = t;
   return st;

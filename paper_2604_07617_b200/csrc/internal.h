@@ -49,6 +49,7 @@ struct TraceArgs {
   const double* script_h;  // [script_len][n]; a particle stops at the first h <= 0
   double* script_r;        // [script_len][n] error ratio of every scripted step (nullable)
   int script_len;
+  double* kall;            // step-once hook: [7][4][n] stage derivatives
 };
 
 void set_error(const std::string& msg);
@@ -73,6 +74,10 @@ catapult_status launch_trace_scripted(const TraceConst& tc, const TraceArgs& a, 
 catapult_status launch_step_once(const TraceConst& tc, int model, int64_t n, const double* d_x, const double* d_t,
                                  const double* d_h, double* d_xnew, double* d_err, double* d_k, cudaStream_t s);
 catapult_status trace_launch_shape(int model, int64_t n, int* blocks, int* threads);
+
+// tracer_split.cu (mode: 0 adaptive, 1 scripted replay, 2 one attempted step)
+catapult_status launch_trace_split(const TraceConst& tc, const TraceArgs& a, int model, int mode, cudaStream_t s);
+catapult_status trace_split_launch_shape(int model, int64_t n, int* blocks, int* threads);
 
 // estimate.cu
 catapult_status launch_estimate(int g_kind, int64_t n, const int* d_status, const double* d_tstop,

@@ -13,7 +13,7 @@ CSRC = os.path.join(PKG, "csrc")
 INC = os.path.join(ROOT, "include")
 LIB = os.path.join(PKG, "libcatapult.so")
 OBJ = os.path.join(PKG, "build")
-SOURCES = ["api.cu", "field.cu", "tracer.cu", "tracer_split.cu", "estimate.cu", "peaks.cu", "mathprobe.cu"]
+SOURCES = ["api.cu", "field.cu", "tracer.cu", "estimate.cu", "peaks.cu", "mathprobe.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-I", INC, "-I", CSRC]
@@ -32,6 +32,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     os.makedirs(OBJ, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
+    extra += os.environ.get("CATAPULT_NVCC_FLAGS", "").split()     # e.g. -DCATAPULT_SPLIT_NREG_BOOZER=24 for sweeps
 
     def compile_one(src):
         obj = os.path.join(OBJ, src.replace(".cu", ".o"))

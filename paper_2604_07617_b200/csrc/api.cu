@@ -2,7 +2,6 @@
 // parameter packing and stream-ordered launches.  No arithmetic of the method lives here.
 #include <cmath>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -106,9 +105,12 @@ static catapult_status make_trace_const(const catapult_field* f, const catapult_
   if (!(dtmax > 0.0)) {
     double L;
     if (f->desc.coord == CATAPULT_COORD_BOOZER) {
-      double b00 = 1.0;  // |B| at the first node = first coefficient of the first cell
-      cudaError_t e = cudaMemcpy(&b00, f->d_table, sizeof(double), cudaMemcpyDeviceToHost);
+      // |B| at the first node = the first cell's polynomial at w = (-1,-1,-1) (gc_device.cuh basis)
+      double c[64];
+      cudaError_t e = cudaMemcpy(c, f->d_table, sizeof(c), cudaMemcpyDeviceToHost);
       if (e != cudaSuccess) return cuda_fail(e, "reading |B|(node 0) for the default dtmax");
+      double b00 = 0.0;
+      for (int i = 0; i < 64; ++i) b00 += (((i >> 4) + ((i >> 2) & 3) + (i & 3)) & 1) ? -c[i] : c[i];
       L = std::fabs(f->desc.G0) / std::fabs(b00);
     } else {
       L = f->desc.hi[0];
@@ -131,12 +133,6 @@ static catapult_status make_trace_const(const catapult_field* f, const catapult_
   *model = f->desc.coord == CATAPULT_COORD_CYL ? MODEL_CART : (p->saw_on ? MODEL_BOOZER_SAW : MODEL_BOOZER_VAC);
   (void)E_CHARGE;
   return CATAPULT_OK;
-}
-
-// CATAPULT_TRACER=group selects the first-generation kernel (4-lane groups, tracer.cu) for A/B runs
-static bool use_group_tracer() {
-  const char* e = std::getenv("CATAPULT_TRACER");
-  return e && std::strcmp(e, "group") == 0;
 }
 
 static catapult_status use_device_of(const catapult_field* f) {
@@ -254,8 +250,7 @@ static catapult_status run_trace(const catapult_field* f, const catapult_trace_p
     return cuda_fail(e, "cudaMemsetAsync(queue)");
   }
   a.queue = queue;
-  if (use_group_tracer()) st = scripted ? launch_trace_scripted(tc, a, model, s) : launch_trace(tc, a, model, s);
-  else st = launch_trace_split(tc, a, model, scripted ? 1 : 0, s);
+  st = launch_trace(tc, a, model, scripted ? 1 : 0, s);
   cudaFreeAsync(queue, s);
   return st;
 }
@@ -447,8 +442,6 @@ catapult_status catapult_step_once(const catapult_field* f, const catapult_trace
   if (st != CATAPULT_OK) return st;
   st = use_device_of(f);
   if (st != CATAPULT_OK) return st;
-  if (use_group_tracer())
-    return launch_step_once(tc, model, n, d_x, d_t, d_h, d_xnew, d_errratio, d_k, (cudaStream_t)stream);
   if (n == 0) return CATAPULT_OK;
   TraceArgs a{};
   a.n = n;
@@ -467,7 +460,7 @@ catapult_status catapult_step_once(const catapult_field* f, const catapult_trace
     return cuda_fail(e, "cudaMemsetAsync(queue)");
   }
   a.queue = queue;
-  st = launch_trace_split(tc, a, model, 2, s);
+  st = launch_trace(tc, a, model, 2, s);
   cudaFreeAsync(queue, s);
   return st;
 }
@@ -515,8 +508,7 @@ catapult_status catapult_trace_launch_shape(const catapult_field* f, const catap
   catapult_status st = make_trace_const(f, p, &tc, &model);
   if (st != CATAPULT_OK) return st;
   int b = 0, t = 0;
-  st = use_group_tracer() ? trace_launch_shape(model, (int64_t)1 << 40, &b, &t)
-                          : trace_split_launch_shape(model, (int64_t)1 << 40, &b, &t);
+  st = trace_launch_shape(model, (int64_t)1 << 40, &b, &t);
   *blocks = b;
   *threads = t;
   return st;

@@ -1,55 +1,105 @@
-// Field-table kernels: unique nodes -> per-cell 64-coefficient tables (PAPER.md:67-69), the
-// tricubic test hook and the export in the paper's own row layout.
+// Field-table kernels: unique nodes -> per-cell 64-coefficient tables (PAPER.md:47-53, 67-69), the
+// tricubic test hook and the export of nodal rows in the paper's own layout.
 #include "gc_device.cuh"
 
 namespace catapult {
 
-// One thread per table element.  out[(cell*m + q)*64 + node], node = (a*4+b)*4+c,
-// value = nodes[q][3*i0+a][3*i1+b][3*i2+c].  Writes are fully coalesced; the reads of a cell's
-// 4-node runs come from L2 (the unique-node array is 64/27 times smaller than the table).
-__global__ void __launch_bounds__(256)
+// ---- double-double helpers (the basis change is done in ~106-bit arithmetic) ---------------------------
+struct dd {
+  double hi, lo;
+};
+__device__ __forceinline__ dd dd_norm(double s, double e) {  // |e| <= |s|
+  const double h = s + e;
+  return dd{h, e - (h - s)};
+}
+__device__ __forceinline__ dd dd_add(dd x, dd y) {
+  const double s = x.hi + y.hi;
+  const double bb = s - x.hi;
+  const double e = ((x.hi - (s - bb)) + (y.hi - bb)) + (x.lo + y.lo);
+  return dd_norm(s, e);
+}
+__device__ __forceinline__ dd dd_neg(dd x) { return dd{-x.hi, -x.lo}; }
+__device__ __forceinline__ dd dd_mul(dd x, double m) {  // m a small integer or a power of two
+  const double p = x.hi * m;
+  const double e = fma(x.hi, m, -p) + x.lo * m;
+  return dd_norm(p, e);
+}
+
+// Nodal values f0..f3 at u = 0, 1/3, 2/3, 1 -> coefficients of 1, w, w^2, w^3 with w = 2u - 1.
+// The matrix is [-1 9 9 -1; 1 -27 27 -1; 9 -9 -9 9; -9 27 -27 9] / 16 (exact small integers).
+__device__ __forceinline__ void nodal_to_monomial(dd& f0, dd& f1, dd& f2, dd& f3) {
+  const dd A = dd_add(f1, f2), S = dd_add(f0, f3);
+  const dd D = dd_add(f2, dd_neg(f1)), E = dd_add(f3, dd_neg(f0));
+  const dd c0 = dd_mul(dd_add(dd_mul(A, 9.0), dd_neg(S)), 0.0625);
+  const dd c1 = dd_mul(dd_add(dd_mul(D, 27.0), dd_neg(E)), 0.0625);
+  const dd c2 = dd_mul(dd_add(S, dd_neg(A)), 0.5625);
+  const dd c3 = dd_mul(dd_add(dd_mul(E, 9.0), dd_neg(dd_mul(D, 27.0))), 0.0625);
+  f0 = c0;
+  f1 = c1;
+  f2 = c2;
+  f3 = c3;
+}
+
+// One thread per (cell, quantity): gathers the 4x4x4 nodal block nodes[q][3*i0+a][3*i1+b][3*i2+c] (shared faces
+// are read by both neighbours), changes basis along the three axes, writes 512 contiguous bytes
+// table[(cell*m + q)*64 + (i*4+j)*4+k].
+__global__ void __launch_bounds__(128)
 field_build_kernel(const double* __restrict__ nodes, double* __restrict__ table, int m, int k0, int k1, int k2) {
-  const long long total = (long long)k0 * k1 * k2 * m * 64;
+  const long long total = (long long)k0 * k1 * k2 * m;
   const long long n1 = 3LL * k1 + 1, n2 = 3LL * k2 + 1, n0 = 3LL * k0 + 1;
   for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < total;
        o += (long long)gridDim.x * blockDim.x) {
-    const int node = (int)(o & 63);
-    const long long cq = o >> 6;
-    const int q = (int)(cq % m);
-    const long long cell = cq / m;
+    const int q = (int)(o % m);
+    const long long cell = o / m;
     const int i2 = (int)(cell % k2);
     const long long r = cell / k2;
     const int i1 = (int)(r % k1);
     const int i0 = (int)(r / k1);
-    const int a = node >> 4, b = (node >> 2) & 3, c = node & 3;
-    const long long j0 = 3LL * i0 + a, j1 = 3LL * i1 + b, j2 = 3LL * i2 + c;
-    table[o] = nodes[(long long)q * n0 * n1 * n2 + (j0 * n1 + j1) * n2 + j2];
+    dd v[64];
+    const double* base = nodes + (long long)q * n0 * n1 * n2;
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+      for (int b = 0; b < 4; ++b)
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+          v[(a * 4 + b) * 4 + c] = dd{base[((3LL * i0 + a) * n1 + (3LL * i1 + b)) * n2 + (3LL * i2 + c)], 0.0};
+#pragma unroll
+    for (int stride = 1; stride <= 16; stride *= 4) {
+#pragma unroll
+      for (int g = 0; g < 16; ++g) {
+        // the 16 lines along this axis: index = lo + hi*4*stride, lo in [0,stride), hi in [0,16/stride)
+        const int e0 = (g % stride) + (g / stride) * 4 * stride;
+        nodal_to_monomial(v[e0], v[e0 + stride], v[e0 + 2 * stride], v[e0 + 3 * stride]);
+      }
+    }
+    double* dst = table + o * 64;
+#pragma unroll
+    for (int e = 0; e < 64; ++e) dst[e] = v[e].hi;  // normalised: hi = fl(hi + lo)
   }
 }
 
-// test hook: the production evaluation path (group of NL lanes per point, coefficients staged through
-// the on-chip cell cache) at arbitrary points
-template <int MODEL>
-__global__ void __launch_bounds__(ModelTraits<MODEL>::NT, ModelTraits<MODEL>::MINB)
+// test hook: tricubic values of all quantities at arbitrary points with the production locate and
+// contraction functions, coefficients read straight from the table
+template <bool BOOZER>
+__global__ void __launch_bounds__(128)
 field_eval_kernel(const __grid_constant__ FieldConst f, long long npts, const double* __restrict__ pts,
                   double* __restrict__ out) {
-  using MT = ModelTraits<MODEL>;
-  extern __shared__ double2 smem[];
-  const Group<MT::NL> g;
-  CellCache<MODEL> cc;
-  cc.init(smem);
-  const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) / MT::NL;
-  if (i >= npts) return;  // group-uniform
-  double u[3], fv[MT::NQ];
-  const long long cell = locate<!MT::CART>(f, pts[i], pts[npts + i], pts[2 * npts + i], u);
-  tricubic_group<MODEL>(f, g, cc, cell, u, fv);
-  if (g.j == 0) {
-#pragma unroll
-    for (int q = 0; q < MT::NQ; ++q) out[(long long)q * npts + i] = fv[q];
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= npts) return;
+  double w[3];
+  const int cell = locate<BOOZER>(f, pts[i], pts[npts + i], pts[2 * npts + i], w);
+  for (int q = 0; q < f.m; ++q) {
+    const double* src = f.table + ((long long)cell * f.m + q) * 64;
+    out[(long long)q * npts + i] = horner64(
+        [&](int e, double& f0, double& f1, double& f2, double& f3) { ldg_f64x4(src + e, f0, f1, f2, f3); }, w[0], w[1],
+        w[2]);
   }
 }
 
-// table [cell][q][64] -> rows [(cell*64+node)][q]  (row = node, column = quantity)
+// test hook: nodal values recovered from the table in the paper's row layout (row = node,
+// column = quantity): out[(cell*64+node)*m + q] = polynomial of (cell,q) at the in-cell node (a,b,c),
+// w = -1, -1/3, 1/3, 1.  Equal to the input nodes up to the rounding of the stored coefficients.
 __global__ void field_export_rows_kernel(const double* __restrict__ table, double* __restrict__ out, int m,
                                          long long ncells) {
   const long long total = ncells * m * 64;
@@ -59,7 +109,11 @@ __global__ void field_export_rows_kernel(const double* __restrict__ table, doubl
     const long long row = o / m;
     const int node = (int)(row & 63);
     const long long cell = row >> 6;
-    out[o] = table[(cell * m + q) * 64 + node];
+    const double* src = table + (cell * m + q) * 64;
+    const double wa = ((node >> 4) * 2 - 3) * (1.0 / 3.0), wb = (((node >> 2) & 3) * 2 - 3) * (1.0 / 3.0),
+                 wc = ((node & 3) * 2 - 3) * (1.0 / 3.0);
+    out[o] = horner64(
+        [&](int e, double& f0, double& f1, double& f2, double& f3) { ldg_f64x4(src + e, f0, f1, f2, f3); }, wa, wb, wc);
   }
 }
 
@@ -71,22 +125,9 @@ static int grid_for(long long total, int threads) {
 
 catapult_status launch_field_build(const catapult_field_desc& d, const double* d_nodes, double* d_table,
                                    cudaStream_t s) {
-  const long long total = (long long)d.ncell[0] * d.ncell[1] * d.ncell[2] * d.nquant * 64;
-  field_build_kernel<<<grid_for(total, 256), 256, 0, s>>>(d_nodes, d_table, d.nquant, d.ncell[0], d.ncell[1],
+  const long long total = (long long)d.ncell[0] * d.ncell[1] * d.ncell[2] * d.nquant;
+  field_build_kernel<<<grid_for(total, 128), 128, 0, s>>>(d_nodes, d_table, d.nquant, d.ncell[0], d.ncell[1],
                                                           d.ncell[2]);
-  CATAPULT_CUDA_TRY(cudaGetLastError());
-  return CATAPULT_OK;
-}
-
-template <int MODEL>
-static catapult_status field_eval_one(const FieldConst& fc, int64_t npts, const double* d_pts, double* d_out,
-                                      cudaStream_t s) {
-  using MT = ModelTraits<MODEL>;
-  CATAPULT_CUDA_TRY(cudaFuncSetAttribute(field_eval_kernel<MODEL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)MT::SMEM_BYTES));
-  const long long per_block = MT::NT / MT::NL;
-  const int blocks = (int)((npts + per_block - 1) / per_block);
-  field_eval_kernel<MODEL><<<blocks, MT::NT, MT::SMEM_BYTES, s>>>(fc, npts, d_pts, d_out);
   CATAPULT_CUDA_TRY(cudaGetLastError());
   return CATAPULT_OK;
 }
@@ -94,8 +135,11 @@ static catapult_status field_eval_one(const FieldConst& fc, int64_t npts, const 
 catapult_status launch_field_eval(const FieldConst& fc, int64_t npts, const double* d_pts, double* d_out,
                                   cudaStream_t s) {
   if (npts == 0) return CATAPULT_OK;
-  if (fc.coord == CATAPULT_COORD_BOOZER) return field_eval_one<MODEL_BOOZER_VAC>(fc, npts, d_pts, d_out, s);
-  return field_eval_one<MODEL_CART>(fc, npts, d_pts, d_out, s);
+  const int blocks = (int)((npts + 127) / 128);
+  if (fc.coord == CATAPULT_COORD_BOOZER) field_eval_kernel<true><<<blocks, 128, 0, s>>>(fc, npts, d_pts, d_out);
+  else field_eval_kernel<false><<<blocks, 128, 0, s>>>(fc, npts, d_pts, d_out);
+  CATAPULT_CUDA_TRY(cudaGetLastError());
+  return CATAPULT_OK;
 }
 
 catapult_status launch_field_export_rows(const FieldConst& fc, int64_t ncells, double* d_out, cudaStream_t s) {

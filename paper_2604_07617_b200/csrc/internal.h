@@ -68,16 +68,9 @@ catapult_status launch_field_eval(const FieldConst& fc, int64_t npts, const doub
                                   cudaStream_t s);
 catapult_status launch_field_export_rows(const FieldConst& fc, int64_t ncells, double* d_out, cudaStream_t s);
 
-// tracer.cu
-catapult_status launch_trace(const TraceConst& tc, const TraceArgs& a, int model, cudaStream_t s);
-catapult_status launch_trace_scripted(const TraceConst& tc, const TraceArgs& a, int model, cudaStream_t s);
-catapult_status launch_step_once(const TraceConst& tc, int model, int64_t n, const double* d_x, const double* d_t,
-                                 const double* d_h, double* d_xnew, double* d_err, double* d_k, cudaStream_t s);
+// tracer.cu (mode: 0 adaptive, 1 scripted replay, 2 one attempted step)
+catapult_status launch_trace(const TraceConst& tc, const TraceArgs& a, int model, int mode, cudaStream_t s);
 catapult_status trace_launch_shape(int model, int64_t n, int* blocks, int* threads);
-
-// tracer_split.cu (mode: 0 adaptive, 1 scripted replay, 2 one attempted step)
-catapult_status launch_trace_split(const TraceConst& tc, const TraceArgs& a, int model, int mode, cudaStream_t s);
-catapult_status trace_split_launch_shape(int model, int64_t n, int* blocks, int* threads);
 
 // estimate.cu
 catapult_status launch_estimate(int g_kind, int64_t n, const int* d_status, const double* d_tstop,

@@ -110,7 +110,7 @@ static catapult_status make_trace_const(const catapult_field* f, const catapult_
       cudaError_t e = cudaMemcpy(c, f->d_table, sizeof(c), cudaMemcpyDeviceToHost);
       if (e != cudaSuccess) return cuda_fail(e, "reading |B|(node 0) for the default dtmax");
       double b00 = 0.0;
-      for (int i = 0; i < 64; ++i) b00 += (((i >> 4) + ((i >> 2) & 3) + (i & 3)) & 1) ? -c[i] : c[i];
+      for (int i = 0; i < 64; ++i) b00 += (((i >> 4) + ((i >> 2) & 3) + (i & 3)) & 1) ? -c[coef_pos(i)] : c[coef_pos(i)];
       L = std::fabs(f->desc.G0) / std::fabs(b00);
     } else {
       L = f->desc.hi[0];

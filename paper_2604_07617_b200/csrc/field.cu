@@ -42,7 +42,7 @@ __device__ __forceinline__ void nodal_to_monomial(dd& f0, dd& f1, dd& f2, dd& f3
 
 // One thread per (cell, quantity): gathers the 4x4x4 nodal block nodes[q][3*i0+a][3*i1+b][3*i2+c] (shared faces
 // are read by both neighbours), changes basis along the three axes, writes 512 contiguous bytes
-// table[(cell*m + q)*64 + (i*4+j)*4+k].
+// table[(cell*m + q)*64 + coef_pos((i*4+j)*4+k)] (gc_device.cuh: register half first, shared half second).
 __global__ void __launch_bounds__(128)
 field_build_kernel(const double* __restrict__ nodes, double* __restrict__ table, int m, int k0, int k1, int k2) {
   const long long total = (long long)k0 * k1 * k2 * m;
@@ -75,7 +75,7 @@ field_build_kernel(const double* __restrict__ nodes, double* __restrict__ table,
     }
     double* dst = table + o * 64;
 #pragma unroll
-    for (int e = 0; e < 64; ++e) dst[e] = v[e].hi;  // normalised: hi = fl(hi + lo)
+    for (int e = 0; e < 64; ++e) dst[coef_pos(e)] = v[e].hi;  // normalised: hi = fl(hi + lo)
   }
 }
 
@@ -92,7 +92,7 @@ field_eval_kernel(const __grid_constant__ FieldConst f, long long npts, const do
   for (int q = 0; q < f.m; ++q) {
     const double* src = f.table + ((long long)cell * f.m + q) * 64;
     out[(long long)q * npts + i] = horner64(
-        [&](int e, double& f0, double& f1, double& f2, double& f3) { ldg_f64x4(src + e, f0, f1, f2, f3); }, w[0], w[1],
+        [&](int e, double& f0, double& f1, double& f2, double& f3) { ldg_f64x4(src + coef_pos(e), f0, f1, f2, f3); }, w[0], w[1],
         w[2]);
   }
 }
@@ -113,7 +113,7 @@ __global__ void field_export_rows_kernel(const double* __restrict__ table, doubl
     const double wa = ((node >> 4) * 2 - 3) * (1.0 / 3.0), wb = (((node >> 2) & 3) * 2 - 3) * (1.0 / 3.0),
                  wc = ((node & 3) * 2 - 3) * (1.0 / 3.0);
     out[o] = horner64(
-        [&](int e, double& f0, double& f1, double& f2, double& f3) { ldg_f64x4(src + e, f0, f1, f2, f3); }, wa, wb, wc);
+        [&](int e, double& f0, double& f1, double& f2, double& f3) { ldg_f64x4(src + coef_pos(e), f0, f1, f2, f3); }, wa, wb, wc);
   }
 }
 

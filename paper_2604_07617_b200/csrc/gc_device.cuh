@@ -28,25 +28,49 @@ __device__ __forceinline__ double wrap_periodic(double xr, double span, double i
 
 // cell index clamped to [0, k-1] and centred local coordinate w = 2 (t - cell) - 1 (|w| > 1 => extrapolation,
 // PAPER.md:79).  The floor is taken by the fp64 -> int32 conversion (saturating; NaN -> 0), clamped in integers.
-__device__ __forceinline__ int cell_and_w(double xr, double invh, int k, double& w) {
+__device__ __forceinline__ int cell_and_w(double xr, double invh, int k, double& w, float& pos) {
   const double t = xr * invh;
   int i = __double2int_rd(t);
   i = min(max(i, 0), k - 1);
   w = fma(2.0, t - (double)i, -1.0);
+  pos = (float)t;  // position in cell units, for the tracer's next-cell guess only
   return i;
 }
+__device__ __forceinline__ int cell_and_w(double xr, double invh, int k, double& w) {
+  float pos;
+  return cell_and_w(xr, invh, k, w, pos);
+}
 
-// x = grid coordinates (dim 0 never periodic; dim 1 periodic for Boozer; dim 2 always periodic)
+// x = grid coordinates (dim 0 never periodic; dim 1 periodic for Boozer; dim 2 always periodic): per-dimension
+// cell indices i[3], centred local coordinates w[3], position in cell units pos[3] (fp32)
 template <bool DIM1_PERIODIC>
-__device__ __forceinline__ int locate(const FieldConst& f, double x0, double x1, double x2, double w[3]) {
-  const int i0 = cell_and_w(x0 - f.lo[0], f.invh[0], f.k[0], w[0]);
+__device__ __forceinline__ void locate3(const FieldConst& f, double x0, double x1, double x2, int i[3], double w[3],
+                                        float pos[3]) {
+  i[0] = cell_and_w(x0 - f.lo[0], f.invh[0], f.k[0], w[0], pos[0]);
   double r1 = x1 - f.lo[1];
   if (DIM1_PERIODIC) r1 = wrap_periodic(r1, f.span[1], f.invspan[1]);
-  const int i1 = cell_and_w(r1, f.invh[1], f.k[1], w[1]);
+  i[1] = cell_and_w(r1, f.invh[1], f.k[1], w[1], pos[1]);
   const double r2 = wrap_periodic(x2 - f.lo[2], f.span[2], f.invspan[2]);
-  const int i2 = cell_and_w(r2, f.invh[2], f.k[2], w[2]);
+  i[2] = cell_and_w(r2, f.invh[2], f.k[2], w[2], pos[2]);
+}
+__device__ __forceinline__ int flat_cell(const FieldConst& f, int i0, int i1, int i2) {
   return (i0 * f.k[1] + i1) * f.k[2] + i2;
 }
+template <bool DIM1_PERIODIC>
+__device__ __forceinline__ int locate(const FieldConst& f, double x0, double x1, double x2, double w[3]) {
+  int i[3];
+  float pos[3];
+  locate3<DIM1_PERIODIC>(f, x0, x1, x2, i, w, pos);
+  return flat_cell(f, i[0], i[1], i[2]);
+}
+
+// Storage order of a (cell, quantity) block of 64 coefficients.  Row (i, j) = the 4 coefficients along k of
+// w0^i w1^j.  The rows j = 0, 1 of the four slabs come first (256 bytes: the half a tracer thread keeps in
+// registers), then the rows j = 2, 3 (256 bytes: the half it keeps in shared memory, fetched by ONE bulk copy).
+__host__ __device__ constexpr int coef_row_pos(int row) {  // row = i*4 + j  ->  offset of its 4 coefficients
+  return ((row & 3) < 2 ? 0 : 32) + ((row >> 2) * 2 + (row & 1)) * 4;
+}
+__host__ __device__ constexpr int coef_pos(int e) { return coef_row_pos(e >> 2) + (e & 3); }  // e = (i*4+j)*4+k
 
 // 256-bit read-only global load (sm_100: LDG.E.256)
 __device__ __forceinline__ void ldg_f64x4(const double* p, double& a, double& b, double& c, double& d) {
@@ -57,19 +81,22 @@ __device__ __forceinline__ void ldg_f64x4(const double* p, double& a, double& b,
 // coefficients e..e+3 (a run along k) from wherever they live (registers, shared memory, global).
 template <class Get4>
 __device__ __forceinline__ double horner64(Get4 get4, double w0, double w1, double w2) {
-  double s[4];
+  // rows are taken from the last (i = 3, j = 3) to the first, each folded into its slab's running Horner value
+  // as soon as it is known and each slab into the total: the rows themselves are independent of one another
+  double total = 0.0;
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    double r[4];
+  for (int i = 3; i >= 0; --i) {
+    double slab = 0.0;
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
+    for (int j = 3; j >= 0; --j) {
       double f0, f1, f2, f3;
       get4((i * 4 + j) * 4, f0, f1, f2, f3);
-      r[j] = fma(fma(fma(f3, w2, f2), w2, f1), w2, f0);
+      const double row = fma(fma(fma(f3, w2, f2), w2, f1), w2, f0);
+      slab = (j == 3) ? row : fma(slab, w1, row);
     }
-    s[i] = fma(fma(fma(r[3], w1, r[2]), w1, r[1]), w1, r[0]);
+    total = (i == 3) ? slab : fma(total, w0, slab);
   }
-  return fma(fma(fma(s[3], w0, s[2]), w0, s[1]), w0, s[0]);
+  return total;
 }
 
 // Boost odeint default step adjuster for dopri5 (S2):

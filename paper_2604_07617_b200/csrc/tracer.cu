@@ -7,7 +7,7 @@
 //     guiding-centre physics, error norm, controller, stop test and refill.  Nothing is replicated:
 //     one warp instruction advances 32 particles.
 //   * NQ CONTRACTION warps: lane l of warp q owns the 64 tricubic coefficients of quantity q of slot l's
-//     current cell, on chip (NREG in registers, the rest in a private conflict-free strip of shared
+//     current cell, on chip (half in registers, half in a private conflict-free run of shared
 //     memory), re-fetched from the cell-major table only when the slot's cell changes.  Per evaluation it
 //     reads the slot's (cell, w) from shared memory, evaluates the 64-coefficient polynomial by nested
 //     Horner (63 FMA, gc_device.cuh) and writes one value back.
@@ -20,12 +20,6 @@
 
 namespace catapult {
 
-#ifndef CATAPULT_SPLIT_NREG_BOOZER
-#define CATAPULT_SPLIT_NREG_BOOZER 32
-#endif
-#ifndef CATAPULT_SPLIT_NREG_CART
-#define CATAPULT_SPLIT_NREG_CART 32
-#endif
 #ifndef CATAPULT_SPLIT_MINB_BOOZER
 #define CATAPULT_SPLIT_MINB_BOOZER 4
 #endif
@@ -54,21 +48,33 @@ struct SplitTraits {
   static constexpr int NQ = CART ? CATAPULT_NQUANT_CYL : CATAPULT_NQUANT_BOOZER;
   static constexpr int NT = 32 * (NQ + 1);   // threads per block
   static constexpr int NCT = 32 * NQ;        // contraction threads per block
-  static constexpr int NREG = CART ? CATAPULT_SPLIT_NREG_CART : CATAPULT_SPLIT_NREG_BOOZER;
-  static constexpr int NSH = 64 - NREG;      // coefficients per contraction thread kept in shared memory
   static constexpr int MINB = CART ? CATAPULT_SPLIT_MINB_CART : CATAPULT_SPLIT_MINB_BOOZER;
-  static_assert(NREG % 4 == 0 && NREG >= 0 && NREG <= 64, "NREG must be a multiple of 4 in [0,64]");
+  // A contraction thread keeps the first 32 stored coefficients of its (cell, quantity) block (the rows j = 0, 1
+  // of every slab, gc_device.cuh coef_row_pos) in registers and the other 32 in a private run of shared
+  // memory: 256 bytes + 16 bytes of padding, so that the 8 lanes of a quarter warp reading 16 bytes each at
+  // the same offset of their runs hit 8 different 16-byte bank groups.
+  static constexpr int STRIP = 272;
   // shared-memory layout (bytes)
-  static constexpr size_t OFF_COEF = 0;                             // double2 [NSH/2][NCT]
-  static constexpr size_t OFF_KS = OFF_COEF + (size_t)NSH * 8 * NCT;  // double [7][4][32]
-  static constexpr size_t OFF_U = OFF_KS + 7 * 4 * 32 * 8;          // double [3][32]
-  static constexpr size_t OFF_FV = OFF_U + 3 * 32 * 8;              // double [NQ][32]
-  static constexpr size_t OFF_CELL = OFF_FV + (size_t)NQ * 32 * 8;  // int    [32]
-  static constexpr size_t SMEM_BYTES = OFF_CELL + 32 * 4;
+  static constexpr size_t OFF_COEF = 0;                              // [NCT] runs of STRIP bytes
+  static constexpr size_t OFF_MBAR = OFF_COEF + (size_t)STRIP * NCT;  // uint64 [NCT]: one mbarrier per thread
+  static constexpr size_t OFF_KS = OFF_MBAR + 8 * NCT;               // double [7][4][32]
+  static constexpr size_t OFF_W = OFF_KS + 7 * 4 * 32 * 8;           // double [3][32]
+  static constexpr size_t OFF_FV = OFF_W + 3 * 32 * 8;               // double [NQ][32]
+  static constexpr size_t OFF_REQ = OFF_FV + (size_t)NQ * 32 * 8;    // int2   [32]: code, flat cell index
+  static constexpr size_t OFF_POS = OFF_REQ + 32 * 8;                // float  [3][32]: position in cell units
+  static constexpr size_t OFF_HINT = OFF_POS + 3 * 32 * 4;           // int    [32]
+  static constexpr size_t OFF_CTL = OFF_HINT + 32 * 4;               // int    [4] (word 0 used)
+  static constexpr size_t SMEM_BYTES = OFF_CTL + 16;
 };
 
-constexpr int CELL_NONE = -1;  // slot has nothing to evaluate this round
-constexpr int CELL_QUIT = -2;  // the scalar warp is done: contraction warps exit
+// Request of a slot: (code, flat cell index), the local coordinates w[3] and -- for the guess only -- the
+// position in cell units (fp32).  code = REQ_NONE: nothing to evaluate.  code >= 0: which point of an attempted step this is (0..5 = the six new stage points c = 1/5,
+// 3/10, 4/5, 8/9, 1, 1; REQ_START = a start point).  The contraction warps use it only to guess the NEXT
+// point's cell.  A block-wide control word says what follows the round: nothing, a hint (the scalar warp's
+// accept/reject decisions, published as soon as they are known), or the end of the kernel.
+constexpr int REQ_NONE = -1, REQ_START = 6;
+constexpr int CTL_PLAIN = 0, CTL_HINT = 1, CTL_QUIT = 2;
+constexpr int HINT_NONE = -2, HINT_ACCEPTED = -1;  // >= 0: rejected, the retry starts in this (flat) cell
 
 __device__ __forceinline__ void bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
@@ -77,53 +83,130 @@ __device__ __forceinline__ void bar_arrive(int id, int nthreads) {
   asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-// 16-byte global -> shared copy that bypasses the register file (LDGSTS); completion is per thread
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+// ---- bulk asynchronous copy global -> shared (the TMA unit's 1-D form) with a thread-private mbarrier -------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned mbar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+// this thread's arrival + the number of bytes the copy issued next will deliver
+__device__ __forceinline__ void mbar_expect_tx(unsigned mbar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* gsrc, unsigned bytes, unsigned mbar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(gsrc), "r"(bytes), "r"(mbar)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned mbar, unsigned parity) {
+  unsigned done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(mbar), "r"(parity)
+        : "memory");
+  } while (!done);
+}
 
 // ---- contraction warps -----------------------------------------------------------------------------
+// Where along the attempted step the next evaluation point lies, relative to this one, in units of
+// (this point - start of the attempt): (c_next - c_this)/c_this for c = 1/5, 3/10, 4/5, 8/9, 1.
+__constant__ float NEXT_POINT_RATIO[8] = {0.5f, 5.0f / 3.0f, 1.0f / 9.0f, 0.125f, 0.0f, 0.0f, 0.0f, 0.0f};
+__device__ __forceinline__ float next_point_ratio(int r) { return NEXT_POINT_RATIO[r & 7]; }
+
+// cell of the point pos + ratio (pos - base), all in cell units (fp32: this is only a guess).  Periodic
+// dimensions: both points lie in [0, k), so the short way round differs from the plain difference by at most k.
 template <int MODEL>
-__device__ __forceinline__ void contraction_warp(const double* __restrict__ table, unsigned char* smem, int q,
-                                                 int lane) {
+__device__ __forceinline__ int guess_cell(const FieldConst& f, const float pos[3], const float base[3], float ratio) {
+  int ni[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    const bool periodic = (d == 2) || (d == 1 && MODEL != MODEL_CART);
+    const float kf = (float)f.k[d];
+    float dd = pos[d] - base[d];
+    if (periodic) dd = dd > 0.5f * kf ? dd - kf : (dd < -0.5f * kf ? dd + kf : dd);
+    float p = fmaf(ratio, dd, pos[d]);
+    if (periodic) p = p >= kf ? p - kf : (p < 0.f ? p + kf : p);
+    ni[d] = min(max(__float2int_rd(p), 0), f.k[d] - 1);
+  }
+  return flat_cell(f, ni[0], ni[1], ni[2]);
+}
+
+template <int MODEL>
+__device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned char* smem, int q, int lane,
+                                                 unsigned long long* counters) {
   using ST = SplitTraits<MODEL>;
-  constexpr int NQ = ST::NQ, NREG = ST::NREG, NCT = ST::NCT, NT = ST::NT;
-  double reg[NREG > 0 ? NREG : 1];
-  double2* sl = reinterpret_cast<double2*>(smem + ST::OFF_COEF) + (q * 32 + lane);  // chunk c at sl[c * NCT]
-  const double* ubuf = reinterpret_cast<const double*>(smem + ST::OFF_U);
+  constexpr int NQ = ST::NQ, NT = ST::NT;
+  const double* __restrict__ table = f.table;
+  double reg[32];
+  unsigned char* strip = smem + ST::OFF_COEF + (size_t)(q * 32 + lane) * ST::STRIP;
+  const double2* sl = reinterpret_cast<const double2*>(strip);  // shared row r (0..7): sl[2r], sl[2r+1]
+  const unsigned strip_s = smem_u32(strip);
+  const unsigned mbar = smem_u32(smem + ST::OFF_MBAR) + 8u * (q * 32 + lane);
+  const double* wbuf = reinterpret_cast<const double*>(smem + ST::OFF_W);
   double* fvbuf = reinterpret_cast<double*>(smem + ST::OFF_FV);
-  const volatile int* cellbuf = reinterpret_cast<const volatile int*>(smem + ST::OFF_CELL);
-  int cached = CELL_NONE;
+  const volatile int2* reqbuf = reinterpret_cast<const volatile int2*>(smem + ST::OFF_REQ);
+  const volatile float* posbuf = reinterpret_cast<const volatile float*>(smem + ST::OFF_POS);
+  const volatile int* hintbuf = reinterpret_cast<const volatile int*>(smem + ST::OFF_HINT);
+  const volatile int* ctlp = reinterpret_cast<const volatile int*>(smem + ST::OFF_CTL);
+  int cached = -1;
+  unsigned phase = 0;    // parity of the mbarrier phase the next wait is for
+  bool pending = false;  // a bulk copy into the strip is in flight
+#ifdef CATAPULT_PF_STATS
+  unsigned long long n_block = 0, n_pref = 0;
+#endif
+  float base[3] = {0.f, 0.f, 0.f};  // start point of the attempted step, in cell units
+  mbar_init(mbar, 1);
+
+  // a cell's 512 contiguous bytes of this lane's quantity: the second half goes global -> shared as ONE bulk
+  // asynchronous copy (no register staging, no per-16-byte requests), the first half lands in its final
+  // registers.  Nothing waits here.
+  auto wait_strip = [&]() {
+    if (pending) {
+      mbar_wait(mbar, phase);
+      phase ^= 1u;
+      pending = false;
+    }
+  };
+  auto issue_loads = [&](int c) {
+    const double* src = table + ((long long)c * NQ + q) * 64;
+    wait_strip();  // a wrong guess may still be landing in the strip: let it finish first
+    mbar_expect_tx(mbar, 256);
+    bulk_g2s(strip_s, src + 32, 256, mbar);
+    pending = true;
+#pragma unroll
+    for (int e = 0; e < 32; e += 4) ldg_f64x4(src + e, reg[e], reg[e + 1], reg[e + 2], reg[e + 3]);
+  };
+
   for (;;) {
     bar_sync(1, NT);
-    const int c = cellbuf[lane];
-    if (c == CELL_QUIT) break;  // warp-uniform
-    if (c >= 0) {
-      if (c != cached) {
-        // a new cell: 512 contiguous bytes of this lane's quantity.  The shared-memory part goes global ->
-        // shared without passing through registers (cp.async), the register part lands in its final
-        // registers, so all 16 requests are in flight together: one memory latency per cell change.
-        const double* src = table + ((long long)c * NQ + q) * 64;
-#pragma unroll
-        for (int e = NREG; e < 64; e += 2) cp_async16(sl + ((e - NREG) / 2) * NCT, src + e);
-#pragma unroll
-        for (int e = 0; e < NREG; e += 4) ldg_f64x4(src + e, reg[e], reg[e + 1], reg[e + 2], reg[e + 3]);
-        cp_async_wait_all();
+    const int ctl = *ctlp;
+    if (ctl == CTL_QUIT) break;  // block-uniform
+    const int code = reqbuf[lane].x;
+    if (code >= 0) {
+      const int c = reqbuf[lane].y;
+      if (c != cached) {  // the guess missed (or there was none): one memory latency, paid by the whole block
+        issue_loads(c);
         cached = c;
+#ifdef CATAPULT_PF_STATS
+        ++n_block;
+#endif
       }
-      const double w0 = ubuf[lane], w1 = ubuf[32 + lane], w2 = ubuf[64 + lane];
-      const double acc = horner64(
+      wait_strip();
+      const double w0 = wbuf[lane], w1 = wbuf[32 + lane], w2 = wbuf[64 + lane];
+      fvbuf[q * 32 + lane] = horner64(
           [&](int e, double& f0, double& f1, double& f2, double& f3) {
-            if (e < NREG) {
-              f0 = reg[e];
-              f1 = reg[e + 1];
-              f2 = reg[e + 2];
-              f3 = reg[e + 3];
+            const int pos = coef_row_pos(e >> 2);  // compile-time after unrolling
+            if (pos < 32) {
+              f0 = reg[pos];
+              f1 = reg[pos + 1];
+              f2 = reg[pos + 2];
+              f3 = reg[pos + 3];
             } else {
-              const double2 v01 = sl[((e - NREG) / 2) * NCT];
-              const double2 v23 = sl[((e - NREG) / 2 + 1) * NCT];
+              const double2 v01 = sl[(pos - 32) / 2];
+              const double2 v23 = sl[(pos - 32) / 2 + 1];
               f0 = v01.x;
               f1 = v01.y;
               f2 = v23.x;
@@ -131,11 +214,56 @@ __device__ __forceinline__ void contraction_warp(const double* __restrict__ tabl
             }
           },
           w0, w1, w2);
-      fvbuf[q * 32 + lane] = acc;
     }
     __syncwarp();
     bar_arrive(2, NT);
+    // ---- while the scalar warp works: guess the next point's cell and start fetching it if it is not the
+    // cell held.  Inside an attempted step: straight-line extrapolation from the step's start point.  After
+    // its last point: the scalar warp's accept/reject decision (hint) -- a rejected step is retried from its
+    // start cell, an accepted one continues about a fifth of a step beyond its end point.  A wrong guess costs
+    // what every cell change cost before (a blocking fetch next round); a right one hides the fetch.
+    int target = cached;
+    float pos[3] = {0.f, 0.f, 0.f};
+    if (code >= 0) {
+#pragma unroll
+      for (int d = 0; d < 3; ++d) pos[d] = posbuf[d * 32 + lane];
+    }
+    if (ctl == CTL_HINT) {
+      bar_sync(3, NT);
+      const int hc = hintbuf[lane];
+      if (code >= 0) {
+        if (hc >= 0) {
+          target = hc;
+        } else if (hc == HINT_ACCEPTED) {
+          target = guess_cell<MODEL>(f, pos, base, 0.2f);
+#pragma unroll
+          for (int d = 0; d < 3; ++d) base[d] = pos[d];
+        }
+      }
+    } else if (code >= 0) {
+      if (code == REQ_START) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) base[d] = pos[d];
+      } else {
+        target = guess_cell<MODEL>(f, pos, base, next_point_ratio(code));
+      }
+    }
+    if (target != cached) {
+#ifdef CATAPULT_PF_STATS
+      ++n_pref;
+#endif
+      issue_loads(target);
+      cached = target;
+    }
   }
+#ifdef CATAPULT_PF_STATS
+  if (counters && q == 0) {  // debugging aid: blocking / guessed fetches of quantity 0 in the two spare status counters
+    atomicAdd(counters + 4, n_block);
+    atomicAdd(counters + 5, n_pref);
+  }
+#else
+  (void)counters;
+#endif
 }
 
 // ---- scalar warp: geometry before the field values are known ------------------------------------------
@@ -145,12 +273,13 @@ struct EvalGeo {
 };
 
 template <int MODEL>
-__device__ __forceinline__ int eval_locate(const TraceConst& tc, const double y[4], double w[3], EvalGeo& g) {
+__device__ __forceinline__ void eval_locate(const TraceConst& tc, const double y[4], int i[3], double w[3],
+                                            float pos[3], EvalGeo& g) {
   const double r2 = fma(y[0], y[0], y[1] * y[1]);
   fm::sqrt_rsqrt(r2, g.a, g.inva);
   g.ang = fm::atan2(y[1], y[0]);
-  if (MODEL == MODEL_CART) return locate<false>(tc.f, g.a, y[2], g.ang, w);
-  return locate<true>(tc.f, g.a, g.ang, y[2], w);
+  if (MODEL == MODEL_CART) locate3<false>(tc.f, g.a, y[2], g.ang, i, w, pos);
+  else locate3<true>(tc.f, g.a, g.ang, y[2], i, w, pos);
 }
 
 // everything of the right-hand side that does not need the interpolated field (overlaps the contraction)
@@ -233,31 +362,55 @@ __device__ __forceinline__ void eval_physics(const TraceConst& tc, const double 
   }
 }
 
-// One lock-step evaluation round of the scalar warp: lanes with `on` evaluate the right-hand side at
-// (t, y); the others publish CELL_NONE.  Must be called by all 32 lanes.
+// One lock-step evaluation round of the scalar warp, in two halves.  eval_publish: lanes with code >= 0 hand
+// (cell indices, w) of the point (t, y) to the contraction warps; the others publish REQ_NONE.  eval_collect:
+// picks up the interpolated values and finishes the right-hand side.  Between the two the caller may do
+// anything that does not need field values (it overlaps the contraction).  All 32 lanes must call both.
 template <int MODEL>
-__device__ __forceinline__ void eval_round(const TraceConst& tc, unsigned char* smem, int lane, bool on, double t,
-                                           const double y[4], double mu, double dy[4], double& modB,
-                                           double& level) {
+__device__ __forceinline__ int eval_publish(const TraceConst& tc, unsigned char* smem, int lane, int code, int ctl,
+                                            double t, const double y[4], EvalGeo& g) {
   using ST = SplitTraits<MODEL>;
-  double* ubuf = reinterpret_cast<double*>(smem + ST::OFF_U);
-  const double* fvbuf = reinterpret_cast<const double*>(smem + ST::OFF_FV);
-  volatile int* cellbuf = reinterpret_cast<volatile int*>(smem + ST::OFF_CELL);
-  EvalGeo g;
+  double* wbuf = reinterpret_cast<double*>(smem + ST::OFF_W);
+  int2* reqbuf = reinterpret_cast<int2*>(smem + ST::OFF_REQ);
+  float* posbuf = reinterpret_cast<float*>(smem + ST::OFF_POS);
+  int i[3];
   double w[3];
-  const int cell = eval_locate<MODEL>(tc, y, w, g);
-  ubuf[lane] = w[0];
-  ubuf[32 + lane] = w[1];
-  ubuf[64 + lane] = w[2];
-  cellbuf[lane] = on ? cell : CELL_NONE;
+  float pos[3];
+  eval_locate<MODEL>(tc, y, i, w, pos, g);
+  const int cell = flat_cell(tc.f, i[0], i[1], i[2]);
+  wbuf[lane] = w[0];
+  wbuf[32 + lane] = w[1];
+  wbuf[64 + lane] = w[2];
+  reqbuf[lane] = make_int2(code, cell);
+#pragma unroll
+  for (int d = 0; d < 3; ++d) posbuf[d * 32 + lane] = pos[d];
+  if (lane == 0) *reinterpret_cast<volatile int*>(smem + ST::OFF_CTL) = ctl;
   __syncwarp();
   bar_arrive(1, ST::NT);
   eval_wave<MODEL>(tc, t, y, g);
+  return cell;
+}
+
+template <int MODEL>
+__device__ __forceinline__ void eval_collect(const TraceConst& tc, unsigned char* smem, int lane, const double y[4],
+                                             double mu, const EvalGeo& g, double dy[4], double& modB,
+                                             double& level) {
+  using ST = SplitTraits<MODEL>;
+  const double* fvbuf = reinterpret_cast<const double*>(smem + ST::OFF_FV);
   bar_sync(2, ST::NT);
   double fv[ST::NQ];
 #pragma unroll
   for (int q = 0; q < ST::NQ; ++q) fv[q] = fvbuf[q * 32 + lane];
   eval_physics<MODEL>(tc, y, mu, g, fv, dy, modB, level);
+}
+
+template <int MODEL>
+__device__ __forceinline__ int eval_round(const TraceConst& tc, unsigned char* smem, int lane, int code, double t,
+                                          const double y[4], double mu, double dy[4], double& modB, double& level) {
+  EvalGeo g;
+  const int cell = eval_publish<MODEL>(tc, smem, lane, code, CTL_PLAIN, t, y, g);
+  eval_collect<MODEL>(tc, smem, lane, y, mu, g, dy, modB, level);
+  return cell;
 }
 
 template <int MODEL, int MODE>
@@ -268,7 +421,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
   const int lane = threadIdx.x & 31;
   const int warp = threadIdx.x >> 5;
   if (warp < ST::NQ) {
-    contraction_warp<MODEL>(tc.f.table, smem, warp, lane);
+    contraction_warp<MODEL>(tc.f, smem, warp, lane, a.counters);
     return;
   }
 
@@ -282,6 +435,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
   long long attempts_left = 0;
   int consecutive = 0, step = 0;
   bool active = false, exhausted = false;
+  int base_cell = 0;  // cell of the current step's start point (where a rejected step is retried)
   unsigned long long c_acc = 0, c_rej = 0, c_eval = 0;
   unsigned c_fin[4] = {0, 0, 0, 0};
 
@@ -324,7 +478,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
     if (__any_sync(FULL, fresh)) {
       // the start point's field values give mu and k1
       double dy0[4], B, level;
-      eval_round<MODEL>(tc, smem, lane, fresh, t, y, 0.0, dy0, B, level);
+      eval_round<MODEL>(tc, smem, lane, fresh ? REQ_START : REQ_NONE, t, y, 0.0, dy0, B, level);
       if (fresh) {
         ++c_eval;
         if (MODE != MODE_STEP_ONCE && a.resume) {
@@ -357,8 +511,9 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
       // k1 with the particle's own mu: the field values are those of the round above; only the physics
       // is redone (mu enters linearly; the geometry is recomputed from y, cheap and rare)
       if (__any_sync(FULL, fresh && active)) {
-        eval_round<MODEL>(tc, smem, lane, fresh && active, t, y, mu, dy0, B, level);
+        const int c0 = eval_round<MODEL>(tc, smem, lane, (fresh && active) ? REQ_START : REQ_NONE, t, y, mu, dy0, B, level);
         if (fresh && active) {
+          base_cell = c0;
           ++c_eval;
 #pragma unroll
           for (int c = 0; c < 4; ++c) ks[c * 32] = dy0[c];
@@ -395,45 +550,76 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
     }
     const bool stepping = active && finish < 0;
     if (__any_sync(FULL, stepping)) {
-      double ys[4], dy[4], B_, level = 0.0;
+      double ys[4], dy[4], P[4], B_, level = 0.0;
+      double epart[4] = {0.0, 0.0, 0.0, 0.0}, invden[4] = {0.0, 0.0, 0.0, 0.0};
+      int cell_end = -1;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        dy[c] = ks[c * 32];  // k1 (first-same-as-last, or the start point's derivative)
+        P[c] = 0.0;
+      }
 #pragma unroll 1
       for (int st = 0; st < 6; ++st) {
-        // stage state: y + h sum_j a[st][j] k_j   (row 5 = b: the new state)
-        double acc[4] = {0.0, 0.0, 0.0, 0.0};
+        // stage state y + h sum_{j<=st} a[st][j] k_j (row 5 = b: the new state); the sum over j < st was
+        // accumulated while the previous contraction ran, the newest derivative enters last
+        const double ad = DP_A[st][st];
 #pragma unroll
-        for (int j = 0; j < 6; ++j) {
-          if (j <= st) {
-            const double aj = DP_A[st][j];
+        for (int c = 0; c < 4; ++c) ys[c] = fma(h, fma(ad, dy[c], P[c]), y[c]);
+        EvalGeo g;
+        cell_end = eval_publish<MODEL>(tc, smem, lane, stepping ? st : REQ_NONE,
+                                       (st == 5 && MODE != MODE_STEP_ONCE) ? CTL_HINT : CTL_PLAIN,
+                                       fma(DP_C[st], h, t), ys, g);
+        // ---- overlaps the contraction ----
+        if (st < 5) {
 #pragma unroll
-            for (int c = 0; c < 4; ++c) acc[c] = fma(aj, ks[(j * 4 + c) * 32], acc[c]);
+          for (int c = 0; c < 4; ++c) P[c] = 0.0;
+#pragma unroll
+          for (int j = 0; j < 5; ++j) {
+            if (j <= st) {
+              const double aj = DP_A[st + 1][j];
+#pragma unroll
+              for (int c = 0; c < 4; ++c) P[c] = fma(aj, ks[(j * 4 + c) * 32], P[c]);
+            }
+          }
+        } else {
+          // PAPER.md:85 Eq. 4, c = (1,1,1,v_total), state and derivative at the start of the
+          // step: everything of the error ratio that does not need the last derivative
+          const double ah = fabs(h);
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            double e = 0.0;
+#pragma unroll
+            for (int j = 0; j < 6; ++j)
+              if (j != 1) e = fma(DP_E[j], ks[(j * 4 + c) * 32], e);
+            epart[c] = e;
+            const double sc = (c == 3) ? tc.atol * tc.vtot : tc.atol;
+            invden[c] = fm::rcp(fma(tc.rtol, fma(ah, fabs(ks[c * 32]), fabs(y[c])), sc));
           }
         }
-#pragma unroll
-        for (int c = 0; c < 4; ++c) ys[c] = fma(h, acc[c], y[c]);
-        eval_round<MODEL>(tc, smem, lane, stepping, fma(DP_C[st], h, t), ys, mu, dy, B_, level);
+        eval_collect<MODEL>(tc, smem, lane, ys, mu, g, dy, B_, level);
 #pragma unroll
         for (int c = 0; c < 4; ++c) ks[((st + 1) * 4 + c) * 32] = dy[c];
+      }
+      double r = 0.0, chk = 0.0;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const double e = fma(DP_E[6], dy[c], epart[c]) * h;
+        const double v = fabs(e) * invden[c];
+        chk += v;
+        r = fmax(r, v);
+      }
+      r = (chk == chk) ? r : chk;  // a non-finite component is a rejection
+      if (MODE != MODE_STEP_ONCE) {
+        // the decision goes to the contraction warps at once: a rejected step is retried from its start cell
+        const bool acc_now = (MODE == MODE_SCRIPT) || (r <= 1.0);
+        reinterpret_cast<volatile int*>(smem + ST::OFF_HINT)[lane] =
+            !stepping ? HINT_NONE : acc_now ? HINT_ACCEPTED : base_cell;
+        __syncwarp();
+        bar_arrive(3, ST::NT);
       }
       if (stepping) {
         c_eval += 6;
         if (attempts_left > 0) --attempts_left;
-        // PAPER.md:85 Eq. 4, c = (1,1,1,v_total), state and derivative at the start of the step
-        double r = 0.0, chk = 0.0;
-        const double ah = fabs(h);
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          double e = 0.0;
-#pragma unroll
-          for (int j = 0; j < 7; ++j)
-            if (j != 1) e = fma(DP_E[j], ks[(j * 4 + c) * 32], e);
-          e *= h;
-          const double sc = (c == 3) ? tc.atol * tc.vtot : tc.atol;
-          const double den = fma(tc.rtol, fma(ah, fabs(ks[c * 32]), fabs(y[c])), sc);
-          const double v = fabs(e) * fm::rcp(den);
-          chk += v;
-          r = fmax(r, v);
-        }
-        r = (chk == chk) ? r : chk;  // a non-finite component is a rejection
         bool accepted;
         double dtn;
         if (MODE == MODE_SCRIPT) {
@@ -472,6 +658,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
               y[c] = ys[c];
               ks[c * 32] = dy[c];  // first-same-as-last
             }
+            base_cell = cell_end;
             // DESIGN.md S5: loss first, then T
             if (is_lost<MODEL>(tc, level)) finish = CATAPULT_ST_LOST;
             else if (MODE != MODE_SCRIPT && t >= tc.T) finish = CATAPULT_ST_REACHED_T;
@@ -499,8 +686,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
 
   // release the contraction warps
   {
-    volatile int* cellbuf = reinterpret_cast<volatile int*>(smem + ST::OFF_CELL);
-    cellbuf[lane] = CELL_QUIT;
+    if (lane == 0) *reinterpret_cast<volatile int*>(smem + ST::OFF_CTL) = CTL_QUIT;
     __syncwarp();
     bar_arrive(1, ST::NT);
   }

@@ -64,7 +64,8 @@ struct SplitTraits {
   static constexpr size_t OFF_POS = OFF_REQ + 32 * 8;                // float  [3][32]: position in cell units
   static constexpr size_t OFF_HINT = OFF_POS + 3 * 32 * 4;           // int    [32]
   static constexpr size_t OFF_CTL = OFF_HINT + 32 * 4;               // int    [4] (word 0 used)
-  static constexpr size_t SMEM_BYTES = OFF_CTL + 16;
+  static constexpr size_t OFF_COLD = OFF_CTL + 16;                   // per-lane bookkeeping: 5 x int64[32] + 8 x int32[32]
+  static constexpr size_t SMEM_BYTES = OFF_COLD + 5 * 256 + 8 * 128;
 };
 
 // Request of a slot: (code, flat cell index), the local coordinates w[3] and -- for the guess only -- the
@@ -110,6 +111,18 @@ __device__ __forceinline__ void mbar_wait(unsigned mbar, unsigned parity) {
   } while (!done);
 }
 
+// the 64 bytes of one slab's two shared rows (j = 2: v[0..3], j = 3: v[4..7]) as one batch of loads
+__device__ __forceinline__ void lds_slab(unsigned addr, double (&v)[8]) {
+  asm volatile(
+      "ld.shared.v2.f64 {%0,%1}, [%8];\n\t"
+      "ld.shared.v2.f64 {%2,%3}, [%8+16];\n\t"
+      "ld.shared.v2.f64 {%4,%5}, [%8+32];\n\t"
+      "ld.shared.v2.f64 {%6,%7}, [%8+48];"
+      : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]), "=d"(v[4]), "=d"(v[5]), "=d"(v[6]), "=d"(v[7])
+      : "r"(addr)
+      : "memory");
+}
+
 // ---- contraction warps -----------------------------------------------------------------------------
 // Where along the attempted step the next evaluation point lies, relative to this one, in units of
 // (this point - start of the attempt): (c_next - c_this)/c_this for c = 1/5, 3/10, 4/5, 8/9, 1.
@@ -142,7 +155,6 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
   const double* __restrict__ table = f.table;
   double reg[32];
   unsigned char* strip = smem + ST::OFF_COEF + (size_t)(q * 32 + lane) * ST::STRIP;
-  const double2* sl = reinterpret_cast<const double2*>(strip);  // shared row r (0..7): sl[2r], sl[2r+1]
   const unsigned strip_s = smem_u32(strip);
   const unsigned mbar = smem_u32(smem + ST::OFF_MBAR) + 8u * (q * 32 + lane);
   const double* wbuf = reinterpret_cast<const double*>(smem + ST::OFF_W);
@@ -150,7 +162,6 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
   const volatile int2* reqbuf = reinterpret_cast<const volatile int2*>(smem + ST::OFF_REQ);
   const volatile float* posbuf = reinterpret_cast<const volatile float*>(smem + ST::OFF_POS);
   const volatile int* hintbuf = reinterpret_cast<const volatile int*>(smem + ST::OFF_HINT);
-  const volatile int* ctlp = reinterpret_cast<const volatile int*>(smem + ST::OFF_CTL);
   int cached = -1;
   unsigned phase = 0;    // parity of the mbarrier phase the next wait is for
   bool pending = false;  // a bulk copy into the strip is in flight
@@ -182,11 +193,13 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
 
   for (;;) {
     bar_sync(1, NT);
-    const int ctl = *ctlp;
-    if (ctl == CTL_QUIT) break;  // block-uniform
-    const int code = reqbuf[lane].x;
+    const long long rq_raw = *reinterpret_cast<const volatile long long*>(reqbuf + lane);  // one 8-byte load
+    const int2 rq = make_int2((int)rq_raw, (int)(rq_raw >> 32));
+    const int ctl = rq.x >> 3;                                  // block-uniform
+    if (ctl == CTL_QUIT) break;
+    const int code = (rq.x & 7) == 7 ? REQ_NONE : (rq.x & 7);
     if (code >= 0) {
-      const int c = reqbuf[lane].y;
+      const int c = rq.y;
       if (c != cached) {  // the guess missed (or there was none): one memory latency, paid by the whole block
         issue_loads(c);
         cached = c;
@@ -196,24 +209,25 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
       }
       wait_strip();
       const double w0 = wbuf[lane], w1 = wbuf[32 + lane], w2 = wbuf[64 + lane];
-      fvbuf[q * 32 + lane] = horner64(
-          [&](int e, double& f0, double& f1, double& f2, double& f3) {
-            const int pos = coef_row_pos(e >> 2);  // compile-time after unrolling
-            if (pos < 32) {
-              f0 = reg[pos];
-              f1 = reg[pos + 1];
-              f2 = reg[pos + 2];
-              f3 = reg[pos + 3];
-            } else {
-              const double2 v01 = sl[(pos - 32) / 2];
-              const double2 v23 = sl[(pos - 32) / 2 + 1];
-              f0 = v01.x;
-              f1 = v01.y;
-              f2 = v23.x;
-              f3 = v23.y;
-            }
-          },
-          w0, w1, w2);
+      // horner64 (gc_device.cuh), same operations in the same order, scheduled by hand around the shared
+      // half: the two shared rows (j = 3, 2) of a slab arrive as ONE batch of four 16-byte loads, issued
+      // before the previous slab's register rows (j = 1, 0) are worked, so one shared-memory latency per
+      // slab overlaps six register FMAs instead of sixteen latencies being exposed one by one
+      double v[8];
+      lds_slab(strip_s + 64 * 3, v);
+      double total = 0.0;
+#pragma unroll
+      for (int i = 3; i >= 0; --i) {
+        const double row3 = fma(fma(fma(v[7], w2, v[6]), w2, v[5]), w2, v[4]);
+        const double row2 = fma(fma(fma(v[3], w2, v[2]), w2, v[1]), w2, v[0]);
+        if (i > 0) lds_slab(strip_s + 64 * (i - 1), v);
+        const int r1 = coef_row_pos(i * 4 + 1), r0 = coef_row_pos(i * 4);
+        const double row1 = fma(fma(fma(reg[r1 + 3], w2, reg[r1 + 2]), w2, reg[r1 + 1]), w2, reg[r1]);
+        const double row0 = fma(fma(fma(reg[r0 + 3], w2, reg[r0 + 2]), w2, reg[r0 + 1]), w2, reg[r0]);
+        const double slab = fma(fma(fma(row3, w1, row2), w1, row1), w1, row0);
+        total = (i == 3) ? slab : fma(total, w0, slab);
+      }
+      fvbuf[q * 32 + lane] = total;
     }
     __syncwarp();
     bar_arrive(2, NT);
@@ -362,6 +376,23 @@ __device__ __forceinline__ void eval_physics(const TraceConst& tc, const double 
   }
 }
 
+// sum_{j < NJ} a[NJ][j] k_j: the part of stage state NJ + 2 (row NJ of DP_A) that is known before k_NJ is
+template <int NJ>
+__device__ __forceinline__ void stage_partial(const double* ks, double P[4]) {
+  double k[NJ][4];
+#pragma unroll
+  for (int j = 0; j < NJ; ++j)
+#pragma unroll
+    for (int c = 0; c < 4; ++c) k[j][c] = ks[(j * 4 + c) * 32];
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    double p = 0.0;
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) p = fma(DP_A[NJ][j], k[j][c], p);
+    P[c] = p;
+  }
+}
+
 // One lock-step evaluation round of the scalar warp, in two halves.  eval_publish: lanes with code >= 0 hand
 // (cell indices, w) of the point (t, y) to the contraction warps; the others publish REQ_NONE.  eval_collect:
 // picks up the interpolated values and finishes the right-hand side.  Between the two the caller may do
@@ -381,10 +412,9 @@ __device__ __forceinline__ int eval_publish(const TraceConst& tc, unsigned char*
   wbuf[lane] = w[0];
   wbuf[32 + lane] = w[1];
   wbuf[64 + lane] = w[2];
-  reqbuf[lane] = make_int2(code, cell);
+  reqbuf[lane] = make_int2((code < 0 ? 7 : code) | (ctl << 3), cell);  // one word: what to do + what follows
 #pragma unroll
   for (int d = 0; d < 3; ++d) posbuf[d * 32 + lane] = pos[d];
-  if (lane == 0) *reinterpret_cast<volatile int*>(smem + ST::OFF_CTL) = ctl;
   __syncwarp();
   bar_arrive(1, ST::NT);
   eval_wave<MODEL>(tc, t, y, g);
@@ -430,14 +460,29 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
   const long long n = a.n;
   double* ks = reinterpret_cast<double*>(smem + ST::OFF_KS) + lane;  // k_j component c at ks[(j*4+c)*32]
   double y[4] = {1.0, 0.0, 0.0, 0.0}, t = 0.0, dt = 0.0, mu = 0.0;
-  long long idx = -1;
-  unsigned nacc = 0, nrej = 0;
-  long long attempts_left = 0;
-  int consecutive = 0, step = 0;
+  // bookkeeping that is touched once per attempted step or once per particle lives in shared memory, not in
+  // registers (the compiler would spill it to local memory, whose reloads sat on the critical path)
+  long long* cold64 = reinterpret_cast<long long*>(smem + ST::OFF_COLD) + lane;
+  unsigned* cold32 = reinterpret_cast<unsigned*>(smem + ST::OFF_COLD + 5 * 256) + lane;
+  long long& idx = cold64[0 * 32];
+  long long& attempts_left = cold64[1 * 32];
+  unsigned long long& c_acc = reinterpret_cast<unsigned long long&>(cold64[2 * 32]);
+  unsigned long long& c_rej = reinterpret_cast<unsigned long long&>(cold64[3 * 32]);
+  unsigned long long& c_eval = reinterpret_cast<unsigned long long&>(cold64[4 * 32]);
+  unsigned& nacc = cold32[0 * 32];
+  unsigned& nrej = cold32[1 * 32];
+  int& consecutive = reinterpret_cast<int&>(cold32[2 * 32]);
+  int& step = reinterpret_cast<int&>(cold32[3 * 32]);
+  unsigned* c_fin = cold32 + 4 * 32;  // c_fin[s] at c_fin[s * 32]
+  idx = -1;
+  attempts_left = 0;
+  c_acc = c_rej = c_eval = 0;
+  nacc = nrej = 0;
+  consecutive = step = 0;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) c_fin[j * 32] = 0;
   bool active = false, exhausted = false;
   int base_cell = 0;  // cell of the current step's start point (where a rejected step is retried)
-  unsigned long long c_acc = 0, c_rej = 0, c_eval = 0;
-  unsigned c_fin[4] = {0, 0, 0, 0};
 
   for (;;) {
     // ---- refill: lanes without a particle pull the next index (one atomic per warp) ------------------
@@ -498,7 +543,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
           if (a.mu_io) a.mu_io[idx] = mu;
           if (a.nacc) a.nacc[idx] = 0;
           if (a.nrej) a.nrej[idx] = 0;
-          ++c_fin[CATAPULT_ST_LOST];
+          ++c_fin[CATAPULT_ST_LOST * 32];
         } else if (MODE != MODE_STEP_ONCE && a.init_only) {
           a.t_io[idx] = 0.0;
           a.status[idx] = CATAPULT_ST_REACHED_T;
@@ -571,15 +616,12 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
                                        fma(DP_C[st], h, t), ys, g);
         // ---- overlaps the contraction ----
         if (st < 5) {
-#pragma unroll
-          for (int c = 0; c < 4; ++c) P[c] = 0.0;
-#pragma unroll
-          for (int j = 0; j < 5; ++j) {
-            if (j <= st) {
-              const double aj = DP_A[st + 1][j];
-#pragma unroll
-              for (int c = 0; c < 4; ++c) P[c] = fma(aj, ks[(j * 4 + c) * 32], P[c]);
-            }
+          switch (st) {  // all the loads of a row first, then its sums (j ascending, as everywhere)
+            case 0: stage_partial<1>(ks, P); break;
+            case 1: stage_partial<2>(ks, P); break;
+            case 2: stage_partial<3>(ks, P); break;
+            case 3: stage_partial<4>(ks, P); break;
+            default: stage_partial<5>(ks, P); break;
           }
         } else {
           // PAPER.md:85 Eq. 4, c = (1,1,1,v_total), state and derivative at the start of the
@@ -679,21 +721,21 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
       if (a.nrej) a.nrej[idx] = (a.resume ? a.nrej[idx] : 0u) + nrej;
       c_acc += nacc;
       c_rej += nrej;
-      ++c_fin[finish];
+      ++c_fin[finish * 32];
       active = false;
     }
   }
 
   // release the contraction warps
   {
-    if (lane == 0) *reinterpret_cast<volatile int*>(smem + ST::OFF_CTL) = CTL_QUIT;
+    reinterpret_cast<int2*>(smem + ST::OFF_REQ)[lane] = make_int2(7 | (CTL_QUIT << 3), 0);
     __syncwarp();
     bar_arrive(1, ST::NT);
   }
 
   // ---- statistics: one atomic per warp per counter -----------------------------------------------------
   if (a.counters) {
-    unsigned long long v[7] = {c_acc, c_rej, c_fin[0], c_fin[1], c_fin[2], c_fin[3], c_eval};
+    unsigned long long v[7] = {c_acc, c_rej, c_fin[0], c_fin[32], c_fin[64], c_fin[96], c_eval};
 #pragma unroll
     for (int j = 0; j < 7; ++j) {
       unsigned long long s = v[j];

@@ -77,26 +77,34 @@ __device__ __forceinline__ void ldg_f64x4(const double* p, double& a, double& b,
   asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
 }
 
-// sum_ijk C[(i*4+j)*4+k] w0^i w1^j w2^k by nested Horner (48 + 12 + 3 FMA).  get4(e, f0..f3) delivers the
-// coefficients e..e+3 (a run along k) from wherever they live (registers, shared memory, global).
+// sum_ijk C[(i*4+j)*4+k] w0^i w1^j w2^k.  get4(e, f0..f3) delivers the coefficients e..e+3 (a run along k) from
+// wherever they live (registers, shared memory, global).  The polynomial is evaluated as U + w1^2 V, where U
+// collects the rows j = 0, 1 and V the rows j = 2, 3 of every slab i (the two halves of the stored block,
+// coef_row_pos): each row by Horner in w2 (3 FMA), the two rows of a slab half by one FMA in w1, the four slabs
+// of a half by Horner in w0, and one last FMA: 48 + 8 + 6 + 1 = 63 FMA and one multiplication.  The two halves
+// are independent of each other, which is what the tracer's contraction warps exploit (tracer.cu); every user
+// of the table evaluates it in this one order.
 template <class Get4>
 __device__ __forceinline__ double horner64(Get4 get4, double w0, double w1, double w2) {
-  // rows are taken from the last (i = 3, j = 3) to the first, each folded into its slab's running Horner value
-  // as soon as it is known and each slab into the total: the rows themselves are independent of one another
-  double total = 0.0;
+  double half[2];
 #pragma unroll
-  for (int i = 3; i >= 0; --i) {
-    double slab = 0.0;
+  for (int hh = 0; hh < 2; ++hh) {
+    double acc = 0.0;
 #pragma unroll
-    for (int j = 3; j >= 0; --j) {
-      double f0, f1, f2, f3;
-      get4((i * 4 + j) * 4, f0, f1, f2, f3);
-      const double row = fma(fma(fma(f3, w2, f2), w2, f1), w2, f0);
-      slab = (j == 3) ? row : fma(slab, w1, row);
+    for (int i = 3; i >= 0; --i) {
+      double row[2];
+#pragma unroll
+      for (int jj = 0; jj < 2; ++jj) {
+        double f0, f1, f2, f3;
+        get4((i * 4 + 2 * hh + jj) * 4, f0, f1, f2, f3);
+        row[jj] = fma(fma(fma(f3, w2, f2), w2, f1), w2, f0);
+      }
+      const double pair = fma(row[1], w1, row[0]);
+      acc = (i == 3) ? pair : fma(acc, w0, pair);
     }
-    total = (i == 3) ? slab : fma(total, w0, slab);
+    half[hh] = acc;
   }
-  return total;
+  return fma(half[1], w1 * w1, half[0]);
 }
 
 // Boost odeint default step adjuster for dopri5 (S2):

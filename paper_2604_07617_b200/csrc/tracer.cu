@@ -29,6 +29,22 @@ namespace catapult {
 
 constexpr int MODE_ADAPTIVE = 0, MODE_SCRIPT = 1, MODE_STEP_ONCE = 2;
 
+#ifdef CATAPULT_PF_STATS
+__device__ unsigned long long g_blk[8];  // debugging aid: blocking fetches by request code
+extern "C" int catapult_debug_blocking(unsigned long long* out8) {
+  return cudaMemcpyFromSymbol(out8, g_blk, sizeof(g_blk)) != cudaSuccess;
+}
+#endif
+#ifdef CATAPULT_TIMELINE
+// debugging aid (not part of the product build): cycle counts of the phases of a round, summed over rounds
+__device__ unsigned long long g_tl[16];
+#define TL_NOW() clock64()
+#define TL_ADD(slot, v) (tl_acc[slot] += (unsigned long long)(v))
+#else
+#define TL_NOW() 0LL
+#define TL_ADD(slot, v) ((void)0)
+#endif
+
 // Dormand-Prince 5(4) tableau for the rolled stage loop (row i = coefficients of the state fed to stage
 // i+2; the last row is b: the 7th stage is evaluated at the new state).  PAPER.md:61, ref [10].
 __constant__ double DP_A[6][6] = {
@@ -61,21 +77,18 @@ struct SplitTraits {
   static constexpr size_t OFF_W = OFF_KS + 7 * 4 * 32 * 8;           // double [3][32]
   static constexpr size_t OFF_FV = OFF_W + 3 * 32 * 8;               // double [NQ][32]
   static constexpr size_t OFF_REQ = OFF_FV + (size_t)NQ * 32 * 8;    // int2   [32]: code, flat cell index
-  static constexpr size_t OFF_POS = OFF_REQ + 32 * 8;                // float  [3][32]: position in cell units
-  static constexpr size_t OFF_HINT = OFF_POS + 3 * 32 * 4;           // int    [32]
-  static constexpr size_t OFF_CTL = OFF_HINT + 32 * 4;               // int    [4] (word 0 used)
-  static constexpr size_t OFF_COLD = OFF_CTL + 16;                   // per-lane bookkeeping: 5 x int64[32] + 8 x int32[32]
-  static constexpr size_t SMEM_BYTES = OFF_COLD + 5 * 256 + 8 * 128;
+  static constexpr size_t OFF_POS = OFF_REQ + 32 * 8;                // float  [2][3][32]: last point, start point (cell units)
+  static constexpr size_t OFF_GUESS = OFF_POS + 2 * 3 * 32 * 4;      // int    [32]: guessed cell of the next point
+  static constexpr size_t OFF_COLD = OFF_GUESS + 32 * 4;                   // per-lane bookkeeping: 5 x int64[32] + 8 x int32[32]
+  static constexpr size_t OFF_TL = OFF_COLD + 5 * 256 + 8 * 128;     // int64 [4]: timestamps of the CATAPULT_TIMELINE build
+  static constexpr size_t SMEM_BYTES = OFF_TL + 32 + 128;
 };
 
-// Request of a slot: (code, flat cell index), the local coordinates w[3] and -- for the guess only -- the
-// position in cell units (fp32).  code = REQ_NONE: nothing to evaluate.  code >= 0: which point of an attempted step this is (0..5 = the six new stage points c = 1/5,
-// 3/10, 4/5, 8/9, 1, 1; REQ_START = a start point).  The contraction warps use it only to guess the NEXT
-// point's cell.  A block-wide control word says what follows the round: nothing, a hint (the scalar warp's
-// accept/reject decisions, published as soon as they are known), or the end of the kernel.
+// Request of a slot: one word (what to evaluate: a stage point 0..5 of an attempted step, a start point, or
+// nothing; whether the kernel ends) + the flat cell index, and the local coordinates w[3].  The guess of the
+// NEXT point's cell travels separately (OFF_GUESS, barrier 3).
 constexpr int REQ_NONE = -1, REQ_START = 6;
-constexpr int CTL_PLAIN = 0, CTL_HINT = 1, CTL_QUIT = 2;
-constexpr int HINT_NONE = -2, HINT_ACCEPTED = -1;  // >= 0: rejected, the retry starts in this (flat) cell
+constexpr int CTL_PLAIN = 0, CTL_QUIT = 2;
 
 __device__ __forceinline__ void bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
@@ -160,15 +173,13 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
   const double* wbuf = reinterpret_cast<const double*>(smem + ST::OFF_W);
   double* fvbuf = reinterpret_cast<double*>(smem + ST::OFF_FV);
   const volatile int2* reqbuf = reinterpret_cast<const volatile int2*>(smem + ST::OFF_REQ);
-  const volatile float* posbuf = reinterpret_cast<const volatile float*>(smem + ST::OFF_POS);
-  const volatile int* hintbuf = reinterpret_cast<const volatile int*>(smem + ST::OFF_HINT);
+  const volatile int* guessbuf = reinterpret_cast<const volatile int*>(smem + ST::OFF_GUESS);
   int cached = -1;
   unsigned phase = 0;    // parity of the mbarrier phase the next wait is for
   bool pending = false;  // a bulk copy into the strip is in flight
 #ifdef CATAPULT_PF_STATS
   unsigned long long n_block = 0, n_pref = 0;
 #endif
-  float base[3] = {0.f, 0.f, 0.f};  // start point of the attempted step, in cell units
   mbar_init(mbar, 1);
 
   // a cell's 512 contiguous bytes of this lane's quantity: the second half goes global -> shared as ONE bulk
@@ -191,8 +202,16 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
     for (int e = 0; e < 32; e += 4) ldg_f64x4(src + e, reg[e], reg[e + 1], reg[e + 2], reg[e + 3]);
   };
 
+  volatile long long* tl = reinterpret_cast<volatile long long*>(smem + ST::OFF_TL);
+  volatile unsigned long long* tl_acc = reinterpret_cast<volatile unsigned long long*>(smem + ST::OFF_TL + 32);
+  (void)tl_acc;
+  const bool tl_on = (q == 0 && lane == 0);
+  long long tl_t0 = TL_NOW();
   for (;;) {
     bar_sync(1, NT);
+    const long long tl_wake = TL_NOW();
+    (void)tl_wake;
+    if (tl_on) { TL_ADD(9, tl_wake - tl_t0); TL_ADD(5, tl_wake - tl[0]); }
     const long long rq_raw = *reinterpret_cast<const volatile long long*>(reqbuf + lane);  // one 8-byte load
     const int2 rq = make_int2((int)rq_raw, (int)(rq_raw >> 32));
     const int ctl = rq.x >> 3;                                  // block-uniform
@@ -205,63 +224,58 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
         cached = c;
 #ifdef CATAPULT_PF_STATS
         ++n_block;
+        if (q == 0) atomicAdd(&g_blk[code & 7], 1ULL);
 #endif
       }
       wait_strip();
       const double w0 = wbuf[lane], w1 = wbuf[32 + lane], w2 = wbuf[64 + lane];
-      // horner64 (gc_device.cuh), same operations in the same order, scheduled by hand around the shared
-      // half: the two shared rows (j = 3, 2) of a slab arrive as ONE batch of four 16-byte loads, issued
-      // before the previous slab's register rows (j = 1, 0) are worked, so one shared-memory latency per
-      // slab overlaps six register FMAs instead of sixteen latencies being exposed one by one
+      // horner64 (gc_device.cuh), same operations in the same order, scheduled by hand: the register half U
+      // (8 independent rows) is worked while the first batch of the shared half is in flight; the shared
+      // half V comes slab by slab, each slab's two rows as ONE batch of four 16-byte loads issued as soon as
+      // the previous batch has been consumed
       double v[8];
       lds_slab(strip_s + 64 * 3, v);
-      double total = 0.0;
+      double U;
+      {
+        double pr[4];
+#pragma unroll
+        for (int g = 0; g < 2; ++g) {  // slabs 3,2 then 1,0: four rows at a time, level by level
+          double a4[4];
+#pragma unroll
+          for (int r = 0; r < 4; ++r) a4[r] = fma(reg[(4 * (1 - g) + r) * 4 + 3], w2, reg[(4 * (1 - g) + r) * 4 + 2]);
+#pragma unroll
+          for (int r = 0; r < 4; ++r) a4[r] = fma(a4[r], w2, reg[(4 * (1 - g) + r) * 4 + 1]);
+#pragma unroll
+          for (int r = 0; r < 4; ++r) a4[r] = fma(a4[r], w2, reg[(4 * (1 - g) + r) * 4]);
+          pr[2 * (1 - g) + 1] = fma(a4[3], w1, a4[2]);  // stored row = i*2 + j
+          pr[2 * (1 - g)] = fma(a4[1], w1, a4[0]);
+        }
+        U = fma(fma(fma(pr[3], w0, pr[2]), w0, pr[1]), w0, pr[0]);
+      }
+      double V = 0.0;
 #pragma unroll
       for (int i = 3; i >= 0; --i) {
-        const double row3 = fma(fma(fma(v[7], w2, v[6]), w2, v[5]), w2, v[4]);
-        const double row2 = fma(fma(fma(v[3], w2, v[2]), w2, v[1]), w2, v[0]);
+        const double row1 = fma(fma(fma(v[7], w2, v[6]), w2, v[5]), w2, v[4]);
+        const double row0 = fma(fma(fma(v[3], w2, v[2]), w2, v[1]), w2, v[0]);
         if (i > 0) lds_slab(strip_s + 64 * (i - 1), v);
-        const int r1 = coef_row_pos(i * 4 + 1), r0 = coef_row_pos(i * 4);
-        const double row1 = fma(fma(fma(reg[r1 + 3], w2, reg[r1 + 2]), w2, reg[r1 + 1]), w2, reg[r1]);
-        const double row0 = fma(fma(fma(reg[r0 + 3], w2, reg[r0 + 2]), w2, reg[r0 + 1]), w2, reg[r0]);
-        const double slab = fma(fma(fma(row3, w1, row2), w1, row1), w1, row0);
-        total = (i == 3) ? slab : fma(total, w0, slab);
+        const double pair = fma(row1, w1, row0);
+        V = (i == 3) ? pair : fma(V, w0, pair);
       }
+      const double total = fma(V, w1 * w1, U);
       fvbuf[q * 32 + lane] = total;
+      if (tl_on) TL_ADD(7, TL_NOW() - tl_h0);
     }
     __syncwarp();
+    const long long tl_a2 = TL_NOW();
+    if (tl_on) tl[1] = tl_a2;
     bar_arrive(2, NT);
-    // ---- while the scalar warp works: guess the next point's cell and start fetching it if it is not the
-    // cell held.  Inside an attempted step: straight-line extrapolation from the step's start point.  After
-    // its last point: the scalar warp's accept/reject decision (hint) -- a rejected step is retried from its
-    // start cell, an accepted one continues about a fifth of a step beyond its end point.  A wrong guess costs
-    // what every cell change cost before (a blocking fetch next round); a right one hides the fetch.
-    int target = cached;
-    float pos[3] = {0.f, 0.f, 0.f};
-    if (code >= 0) {
-#pragma unroll
-      for (int d = 0; d < 3; ++d) pos[d] = posbuf[d * 32 + lane];
-    }
-    if (ctl == CTL_HINT) {
-      bar_sync(3, NT);
-      const int hc = hintbuf[lane];
-      if (code >= 0) {
-        if (hc >= 0) {
-          target = hc;
-        } else if (hc == HINT_ACCEPTED) {
-          target = guess_cell<MODEL>(f, pos, base, 0.2f);
-#pragma unroll
-          for (int d = 0; d < 3; ++d) base[d] = pos[d];
-        }
-      }
-    } else if (code >= 0) {
-      if (code == REQ_START) {
-#pragma unroll
-        for (int d = 0; d < 3; ++d) base[d] = pos[d];
-      } else {
-        target = guess_cell<MODEL>(f, pos, base, next_point_ratio(code));
-      }
-    }
+    // ---- while the scalar warp works: it publishes its guess of the NEXT point's cell (barrier 3: in its
+    // overlap window inside an attempted step; right after the accept/reject decision at its end); start
+    // fetching that cell if it is not the one held.  A wrong guess costs what every cell change cost before
+    // (a blocking fetch next round); a right one hides the fetch entirely.
+    bar_sync(3, NT);
+    int target = guessbuf[lane];
+    if (code < 0 || target < 0) target = cached;
     if (target != cached) {
 #ifdef CATAPULT_PF_STATS
       ++n_pref;
@@ -269,6 +283,8 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
       issue_loads(target);
       cached = target;
     }
+    tl_t0 = TL_NOW();
+    if (tl_on) TL_ADD(8, tl_t0 - tl_a2);
   }
 #ifdef CATAPULT_PF_STATS
   if (counters && q == 0) {  // debugging aid: blocking / guessed fetches of quantity 0 in the two spare status counters
@@ -398,15 +414,14 @@ __device__ __forceinline__ void stage_partial(const double* ks, double P[4]) {
 // picks up the interpolated values and finishes the right-hand side.  Between the two the caller may do
 // anything that does not need field values (it overlaps the contraction).  All 32 lanes must call both.
 template <int MODEL>
-__device__ __forceinline__ int eval_publish(const TraceConst& tc, unsigned char* smem, int lane, int code, int ctl,
-                                            double t, const double y[4], EvalGeo& g) {
+__device__ __forceinline__ void eval_publish(const TraceConst& tc, unsigned char* smem, int lane, int code, int ctl,
+                                             double t, const double y[4], EvalGeo& g, float pos[3]) {
   using ST = SplitTraits<MODEL>;
   double* wbuf = reinterpret_cast<double*>(smem + ST::OFF_W);
   int2* reqbuf = reinterpret_cast<int2*>(smem + ST::OFF_REQ);
   float* posbuf = reinterpret_cast<float*>(smem + ST::OFF_POS);
   int i[3];
   double w[3];
-  float pos[3];
   eval_locate<MODEL>(tc, y, i, w, pos, g);
   const int cell = flat_cell(tc.f, i[0], i[1], i[2]);
   wbuf[lane] = w[0];
@@ -416,9 +431,25 @@ __device__ __forceinline__ int eval_publish(const TraceConst& tc, unsigned char*
 #pragma unroll
   for (int d = 0; d < 3; ++d) posbuf[d * 32 + lane] = pos[d];
   __syncwarp();
+#ifdef CATAPULT_TIMELINE
+  {
+    volatile long long* tl = reinterpret_cast<volatile long long*>(smem + ST::OFF_TL);
+    volatile unsigned long long* tl_acc = reinterpret_cast<volatile unsigned long long*>(smem + ST::OFF_TL + 32);
+    const long long now = TL_NOW();
+    if (lane == 0) { TL_ADD(0, 1); TL_ADD(1, now - tl[2]); tl[0] = now; }
+  }
+#endif
   bar_arrive(1, ST::NT);
   eval_wave<MODEL>(tc, t, y, g);
-  return cell;
+}
+
+// the scalar warp's guess of the next evaluation point's cell (-1: none), handed over through barrier 3
+template <int MODEL>
+__device__ __forceinline__ void publish_guess(unsigned char* smem, int lane, int target) {
+  using ST = SplitTraits<MODEL>;
+  reinterpret_cast<volatile int*>(smem + ST::OFF_GUESS)[lane] = target;
+  __syncwarp();
+  bar_arrive(3, ST::NT);
 }
 
 template <int MODEL>
@@ -427,7 +458,19 @@ __device__ __forceinline__ void eval_collect(const TraceConst& tc, unsigned char
                                              double& level) {
   using ST = SplitTraits<MODEL>;
   const double* fvbuf = reinterpret_cast<const double*>(smem + ST::OFF_FV);
+#ifdef CATAPULT_TIMELINE
+  volatile long long* tl = reinterpret_cast<volatile long long*>(smem + ST::OFF_TL);
+  volatile unsigned long long* tl_acc = reinterpret_cast<volatile unsigned long long*>(smem + ST::OFF_TL + 32);
+  const long long tl_b = TL_NOW();
+  if (lane == 0) TL_ADD(2, tl_b - tl[0]);
+#endif
   bar_sync(2, ST::NT);
+#ifdef CATAPULT_TIMELINE
+  {
+    const long long now = TL_NOW();
+    if (lane == 0) { TL_ADD(3, now - tl_b); TL_ADD(4, now - tl[1]); tl[2] = now; }
+  }
+#endif
   double fv[ST::NQ];
 #pragma unroll
   for (int q = 0; q < ST::NQ; ++q) fv[q] = fvbuf[q * 32 + lane];
@@ -435,12 +478,19 @@ __device__ __forceinline__ void eval_collect(const TraceConst& tc, unsigned char
 }
 
 template <int MODEL>
-__device__ __forceinline__ int eval_round(const TraceConst& tc, unsigned char* smem, int lane, int code, double t,
-                                          const double y[4], double mu, double dy[4], double& modB, double& level) {
+__device__ __forceinline__ void eval_round(const TraceConst& tc, unsigned char* smem, int lane, int code, double t,
+                                           const double y[4], double mu, double dy[4], double& modB, double& level) {
+  using ST = SplitTraits<MODEL>;
   EvalGeo g;
-  const int cell = eval_publish<MODEL>(tc, smem, lane, code, CTL_PLAIN, t, y, g);
+  float pos[3];
+  eval_publish<MODEL>(tc, smem, lane, code, CTL_PLAIN, t, y, g, pos);
+  if (code >= 0) {  // a start point: the next attempted step is extrapolated from here
+    float* basebuf = reinterpret_cast<float*>(smem + ST::OFF_POS) + 96;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) basebuf[d * 32 + lane] = pos[d];
+  }
+  publish_guess<MODEL>(smem, lane, -1);
   eval_collect<MODEL>(tc, smem, lane, y, mu, g, dy, modB, level);
-  return cell;
 }
 
 template <int MODEL, int MODE>
@@ -450,8 +500,18 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
   extern __shared__ __align__(16) unsigned char smem[];
   const int lane = threadIdx.x & 31;
   const int warp = threadIdx.x >> 5;
+#ifdef CATAPULT_TIMELINE
+  if (threadIdx.x < 16) reinterpret_cast<unsigned long long*>(smem + ST::OFF_TL + 32)[threadIdx.x] = 0;
+  if (threadIdx.x < 4) reinterpret_cast<long long*>(smem + ST::OFF_TL)[threadIdx.x] = clock64();
+  __syncthreads();
+#endif
   if (warp < ST::NQ) {
     contraction_warp<MODEL>(tc.f, smem, warp, lane, a.counters);
+#ifdef CATAPULT_TIMELINE
+    if (warp == 0 && lane == 0)
+      for (int j = 5; j < 10; ++j)
+        atomicAdd(&g_tl[j], reinterpret_cast<unsigned long long*>(smem + ST::OFF_TL + 32)[j]);
+#endif
     return;
   }
 
@@ -482,7 +542,6 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
 #pragma unroll
   for (int j = 0; j < 4; ++j) c_fin[j * 32] = 0;
   bool active = false, exhausted = false;
-  int base_cell = 0;  // cell of the current step's start point (where a rejected step is retried)
 
   for (;;) {
     // ---- refill: lanes without a particle pull the next index (one atomic per warp) ------------------
@@ -556,9 +615,8 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
       // k1 with the particle's own mu: the field values are those of the round above; only the physics
       // is redone (mu enters linearly; the geometry is recomputed from y, cheap and rare)
       if (__any_sync(FULL, fresh && active)) {
-        const int c0 = eval_round<MODEL>(tc, smem, lane, (fresh && active) ? REQ_START : REQ_NONE, t, y, mu, dy0, B, level);
+        eval_round<MODEL>(tc, smem, lane, (fresh && active) ? REQ_START : REQ_NONE, t, y, mu, dy0, B, level);
         if (fresh && active) {
-          base_cell = c0;
           ++c_eval;
 #pragma unroll
           for (int c = 0; c < 4; ++c) ks[c * 32] = dy0[c];
@@ -597,7 +655,6 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
     if (__any_sync(FULL, stepping)) {
       double ys[4], dy[4], P[4], B_, level = 0.0;
       double epart[4] = {0.0, 0.0, 0.0, 0.0}, invden[4] = {0.0, 0.0, 0.0, 0.0};
-      int cell_end = -1;
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         dy[c] = ks[c * 32];  // k1 (first-same-as-last, or the start point's derivative)
@@ -611,10 +668,20 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
 #pragma unroll
         for (int c = 0; c < 4; ++c) ys[c] = fma(h, fma(ad, dy[c], P[c]), y[c]);
         EvalGeo g;
-        cell_end = eval_publish<MODEL>(tc, smem, lane, stepping ? st : REQ_NONE,
-                                       (st == 5 && MODE != MODE_STEP_ONCE) ? CTL_HINT : CTL_PLAIN,
-                                       fma(DP_C[st], h, t), ys, g);
+        float pos[3];
+        eval_publish<MODEL>(tc, smem, lane, stepping ? st : REQ_NONE, CTL_PLAIN, fma(DP_C[st], h, t), ys, g, pos);
         // ---- overlaps the contraction ----
+        if (st < 5 || MODE == MODE_STEP_ONCE) {
+          // the next point's cell, guessed by straight-line extrapolation from the step's start point (fp32,
+          // cell units): the contraction warps start fetching it as soon as they are done with this point
+          int target = -1;
+          if (stepping && st < 5) {
+            const float* basebuf = reinterpret_cast<const float*>(smem + ST::OFF_POS) + 96;
+            const float base[3] = {basebuf[lane], basebuf[32 + lane], basebuf[64 + lane]};
+            target = guess_cell<MODEL>(tc.f, pos, base, next_point_ratio(st));
+          }
+          publish_guess<MODEL>(smem, lane, target);
+        }
         if (st < 5) {
           switch (st) {  // all the loads of a row first, then its sums (j ascending, as everywhere)
             case 0: stage_partial<1>(ks, P); break;
@@ -651,27 +718,42 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
         r = fmax(r, v);
       }
       r = (chk == chk) ? r : chk;  // a non-finite component is a rejection
+      bool accepted = false;
+      double dtn = h;
+      if (MODE == MODE_SCRIPT) accepted = true;
+      else if (MODE == MODE_ADAPTIVE) dtn = controller(h, r, tc.dtmax, accepted);
       if (MODE != MODE_STEP_ONCE) {
-        // the decision goes to the contraction warps at once: a rejected step is retried from its start cell
-        const bool acc_now = (MODE == MODE_SCRIPT) || (r <= 1.0);
-        reinterpret_cast<volatile int*>(smem + ST::OFF_HINT)[lane] =
-            !stepping ? HINT_NONE : acc_now ? HINT_ACCEPTED : base_cell;
-        __syncwarp();
-        bar_arrive(3, ST::NT);
+        // the decision goes to the contraction warps at once, with the length of the next attempt over this
+        // one's: they guess the cell of its first point (a rejected step is retried from the start point)
+        double hn = h;
+        if (MODE == MODE_ADAPTIVE) {
+          const double tn = accepted ? (clamped ? tc.T : t + h) : t;
+          hn = fmin((accepted && clamped) ? dt : dtn, tc.T - tn);
+        }
+        // first point of the next attempt: end point + ratio (end - start); accepted: a fifth of the next
+        // step over this one beyond the end point, which becomes the new start point; rejected: the same,
+        // measured from the start point
+        const float fr = 0.2f * __fdividef((float)hn, (float)h);
+        int target = -1;
+        if (stepping) {
+          float* posbuf = reinterpret_cast<float*>(smem + ST::OFF_POS);
+          const float pe[3] = {posbuf[lane], posbuf[32 + lane], posbuf[64 + lane]};
+          const float base[3] = {posbuf[96 + lane], posbuf[128 + lane], posbuf[160 + lane]};
+          target = guess_cell<MODEL>(tc.f, pe, base, accepted ? fr : fr - 1.0f);
+          if (accepted) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) posbuf[96 + d * 32 + lane] = pe[d];
+          }
+        }
+        publish_guess<MODEL>(smem, lane, target);
       }
       if (stepping) {
         c_eval += 6;
         if (attempts_left > 0) --attempts_left;
-        bool accepted;
-        double dtn;
         if (MODE == MODE_SCRIPT) {
           if (a.script_r) a.script_r[(long long)step * n + idx] = r;
           ++step;
-          accepted = true;
-          dtn = h;
         } else if (MODE == MODE_STEP_ONCE) {
-          accepted = false;
-          dtn = h;
           double xn[4];
           y_to_state<MODEL>(ys, xn);
 #pragma unroll
@@ -682,8 +764,6 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
 #pragma unroll
             for (int c = 0; c < 4; ++c) a.kall[((long long)j * 4 + c) * n + idx] = ks[(j * 4 + c) * 32];
           active = false;
-        } else {
-          dtn = controller(h, r, tc.dtmax, accepted);
         }
         if (MODE != MODE_STEP_ONCE) {
           if (!accepted) {
@@ -700,7 +780,6 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
               y[c] = ys[c];
               ks[c * 32] = dy[c];  // first-same-as-last
             }
-            base_cell = cell_end;
             // DESIGN.md S5: loss first, then T
             if (is_lost<MODEL>(tc, level)) finish = CATAPULT_ST_LOST;
             else if (MODE != MODE_SCRIPT && t >= tc.T) finish = CATAPULT_ST_REACHED_T;
@@ -733,6 +812,10 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
     bar_arrive(1, ST::NT);
   }
 
+#ifdef CATAPULT_TIMELINE
+  if (lane == 0)
+    for (int j = 0; j < 5; ++j) atomicAdd(&g_tl[j], reinterpret_cast<unsigned long long*>(smem + ST::OFF_TL + 32)[j]);
+#endif
   // ---- statistics: one atomic per warp per counter -----------------------------------------------------
   if (a.counters) {
     unsigned long long v[7] = {c_acc, c_rej, c_fin[0], c_fin[32], c_fin[64], c_fin[96], c_eval};
@@ -797,6 +880,17 @@ catapult_status launch_trace(const TraceConst& tc, const TraceArgs& a, int model
     default: return split_dispatch<MODE_STEP_ONCE>(tc, a, model, s);
   }
 }
+
+#ifdef CATAPULT_TIMELINE
+extern "C" int catapult_debug_timeline(unsigned long long* out16, int reset) {
+  if (out16 && cudaMemcpyFromSymbol(out16, g_tl, sizeof(g_tl)) != cudaSuccess) return 1;
+  if (reset) {
+    unsigned long long z[16] = {0};
+    if (cudaMemcpyToSymbol(g_tl, z, sizeof(z)) != cudaSuccess) return 1;
+  }
+  return 0;
+}
+#endif
 
 catapult_status trace_launch_shape(int model, int64_t n, int* blocks, int* threads) {
   switch (model) {

@@ -16,6 +16,8 @@
 // everything that does not need field values (the wave's exp / sincos); then it picks up the NQ values.
 // The seven stage derivatives live in shared memory, so the stage loop is rolled (one copy of the
 // right-hand side in the instruction stream).
+#include <cstdlib>
+
 #include "gc_device.cuh"
 
 namespace catapult {
@@ -79,7 +81,9 @@ struct SplitTraits {
   static constexpr size_t OFF_REQ = OFF_FV + (size_t)NQ * 32 * 8;    // int2   [32]: code, flat cell index
   static constexpr size_t OFF_POS = OFF_REQ + 32 * 8;                // float  [2][3][32]: last point, start point (cell units)
   static constexpr size_t OFF_GUESS = OFF_POS + 2 * 3 * 32 * 4;      // int    [32]: guessed cell of the next point
-  static constexpr size_t OFF_COLD = OFF_GUESS + 32 * 4;                   // per-lane bookkeeping: 5 x int64[32] + 8 x int32[32]
+  static constexpr size_t OFF_ERR = OFF_GUESS + 32 * 4;               // double [8][32]: known part of the error ratio
+  static constexpr size_t OFF_Y = OFF_ERR + 8 * 32 * 8;               // double [9][32]: state y at the start of the step, dt, stage partial sums
+  static constexpr size_t OFF_COLD = OFF_Y + 9 * 32 * 8;                   // per-lane bookkeeping: 5 x int64[32] + 8 x int32[32]
   static constexpr size_t OFF_TL = OFF_COLD + 5 * 256 + 8 * 128;     // int64 [4]: timestamps of the CATAPULT_TIMELINE build
   static constexpr size_t SMEM_BYTES = OFF_TL + 32 + 128;
 };
@@ -394,18 +398,16 @@ __device__ __forceinline__ void eval_physics(const TraceConst& tc, const double 
 
 // sum_{j < NJ} a[NJ][j] k_j: the part of stage state NJ + 2 (row NJ of DP_A) that is known before k_NJ is
 template <int NJ>
-__device__ __forceinline__ void stage_partial(const double* ks, double P[4]) {
-  double k[NJ][4];
-#pragma unroll
-  for (int j = 0; j < NJ; ++j)
-#pragma unroll
-    for (int c = 0; c < 4; ++c) k[j][c] = ks[(j * 4 + c) * 32];
+__device__ __forceinline__ void stage_partial(const double* ks, double* P) {  // P: shared, stride 32
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
+    double k[NJ];
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) k[j] = ks[(j * 4 + c) * 32];  // the loads of a component first, then its sum
     double p = 0.0;
 #pragma unroll
-    for (int j = 0; j < NJ; ++j) p = fma(DP_A[NJ][j], k[j][c], p);
-    P[c] = p;
+    for (int j = 0; j < NJ; ++j) p = fma(DP_A[NJ][j], k[j], p);
+    P[c * 32] = p;
   }
 }
 
@@ -519,7 +521,10 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
   const unsigned FULL = 0xffffffffu;
   const long long n = a.n;
   double* ks = reinterpret_cast<double*>(smem + ST::OFF_KS) + lane;  // k_j component c at ks[(j*4+c)*32]
-  double y[4] = {1.0, 0.0, 0.0, 0.0}, t = 0.0, dt = 0.0, mu = 0.0;
+  double t = 0.0, mu = 0.0;
+  double* ysm = reinterpret_cast<double*>(smem + ST::OFF_Y) + lane;  // y_c of the step's start at ysm[c * 32]
+  double& dt = ysm[4 * 32];
+  dt = 0.0;
   // bookkeeping that is touched once per attempted step or once per particle lives in shared memory, not in
   // registers (the compiler would spill it to local memory, whose reloads sat on the critical path)
   long long* cold64 = reinterpret_cast<long long*>(smem + ST::OFF_COLD) + lane;
@@ -548,7 +553,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
     const bool want = !active && !exhausted;
     const unsigned need = __ballot_sync(FULL, want);
     bool fresh = false;
-    double x[4] = {0.0, 0.0, 0.0, 0.0};
+    double x[4] = {0.0, 0.0, 0.0, 0.0}, y[4] = {1.0, 0.0, 0.0, 0.0};
     if (need) {
       const int leader = __ffs(need) - 1;
       unsigned long long base = 0;
@@ -619,7 +624,10 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
         if (fresh && active) {
           ++c_eval;
 #pragma unroll
-          for (int c = 0; c < 4; ++c) ks[c * 32] = dy0[c];
+          for (int c = 0; c < 4; ++c) {
+            ks[c * 32] = dy0[c];
+            ysm[c * 32] = y[c];
+          }
           nacc = 0;
           nrej = 0;
           consecutive = 0;
@@ -653,12 +661,13 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
     }
     const bool stepping = active && finish < 0;
     if (__any_sync(FULL, stepping)) {
-      double ys[4], dy[4], P[4], B_, level = 0.0;
-      double epart[4] = {0.0, 0.0, 0.0, 0.0}, invden[4] = {0.0, 0.0, 0.0, 0.0};
+      double ys[4], dy[4], B_, level = 0.0;
+      double* P = ysm + 5 * 32;  // sum_{j<st} a[st][j] k_j of the next stage, written in the overlap window
+      double* errbuf = reinterpret_cast<double*>(smem + ST::OFF_ERR) + lane;  // [c]: sum, [4 + c]: 1/denominator
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         dy[c] = ks[c * 32];  // k1 (first-same-as-last, or the start point's derivative)
-        P[c] = 0.0;
+        P[c * 32] = 0.0;
       }
 #pragma unroll 1
       for (int st = 0; st < 6; ++st) {
@@ -666,7 +675,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
         // accumulated while the previous contraction ran, the newest derivative enters last
         const double ad = DP_A[st][st];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) ys[c] = fma(h, fma(ad, dy[c], P[c]), y[c]);
+        for (int c = 0; c < 4; ++c) ys[c] = fma(h, fma(ad, dy[c], P[c * 32]), ysm[c * 32]);
         EvalGeo g;
         float pos[3];
         eval_publish<MODEL>(tc, smem, lane, stepping ? st : REQ_NONE, CTL_PLAIN, fma(DP_C[st], h, t), ys, g, pos);
@@ -700,9 +709,9 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
 #pragma unroll
             for (int j = 0; j < 6; ++j)
               if (j != 1) e = fma(DP_E[j], ks[(j * 4 + c) * 32], e);
-            epart[c] = e;
+            errbuf[c * 32] = e;
             const double sc = (c == 3) ? tc.atol * tc.vtot : tc.atol;
-            invden[c] = fm::rcp(fma(tc.rtol, fma(ah, fabs(ks[c * 32]), fabs(y[c])), sc));
+            errbuf[(4 + c) * 32] = fm::rcp(fma(tc.rtol, fma(ah, fabs(ks[c * 32]), fabs(ysm[c * 32])), sc));
           }
         }
         eval_collect<MODEL>(tc, smem, lane, ys, mu, g, dy, B_, level);
@@ -712,8 +721,8 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
       double r = 0.0, chk = 0.0;
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
-        const double e = fma(DP_E[6], dy[c], epart[c]) * h;
-        const double v = fabs(e) * invden[c];
+        const double e = fma(DP_E[6], dy[c], errbuf[c * 32]) * h;
+        const double v = fabs(e) * errbuf[(4 + c) * 32];
         chk += v;
         r = fmax(r, v);
       }
@@ -777,7 +786,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
             if (!clamped) dt = dtn;
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-              y[c] = ys[c];
+              ysm[c * 32] = ys[c];
               ks[c * 32] = dy[c];  // first-same-as-last
             }
             // DESIGN.md S5: loss first, then T
@@ -789,7 +798,8 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
     }
     if (active && finish >= 0) {
       double xo[4];
-      y_to_state<MODEL>(y, xo);
+      const double yf[4] = {ysm[0], ysm[32], ysm[64], ysm[96]};
+      y_to_state<MODEL>(yf, xo);
 #pragma unroll
       for (int c = 0; c < 4; ++c) a.x_out[c * n + idx] = xo[c];
       a.t_io[idx] = t;
@@ -843,6 +853,10 @@ static catapult_status split_shape(int64_t n, int* blocks, int* threads) {
   if (per_sm < 1) {
     set_error("the tracer kernel does not fit on this device (registers / shared memory)");
     return CATAPULT_ECUDA;
+  }
+  if (const char* e = getenv("CATAPULT_BLOCKS_PER_SM")) {  // experiments only
+    const int v = atoi(e);
+    if (v >= 1 && v < per_sm) per_sm = v;
   }
   const long long resident = (long long)sms * per_sm;  // persistent: a multiple of the SM count
   long long want = (n + 31) / 32;

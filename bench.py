@@ -278,7 +278,7 @@ def main():
                 "frac": achieved / peak,
                 "peak_source": "measured DFMA micro-benchmark (catapult_measure_fp64_peak)" if peak_fp64 else
                 "nominal 148 SM x 64 DFMA/clk x 1.965 GHz",
-                "traffic": None,
+                "traffic": _ncu_traffic(model, cnt[6] / max(1, args.steps)),
                 "flops_per_rhs_eval": FLOPS_PER_EVAL[model], "rhs_evals_per_launch": cnt[6] / max(1, args.steps),
                 "launch_ms": sum(trace_ms) / max(1, len(trace_ms)),
                 "trace_share_of_step": sum(trace_ms) / ms,
@@ -359,6 +359,22 @@ def main():
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def _ncu_traffic(model: str, evals_per_launch: float):
+    """DRAM bytes of one trace launch: `dram__bytes_read.sum + dram__bytes_write.sum` per right-hand-side
+    evaluation of the committed `ncu --set full` capture (profiles/r1_traffic_v4.md; cfg4 recipe) times the
+    evaluations of one timed launch.  None for the models that were not captured."""
+    if model != "boozer_saw":
+        return None
+    try:
+        for line in open(os.path.join(ROOT, "profiles", "r1_traffic_v4.csv")):
+            f = line.strip().split(",")
+            if f[0] == "dram_bytes_per_rhs_eval":
+                return float(f[1]) * evals_per_launch
+    except Exception:
+        pass
+    return None
 
 
 def _measured_peaks() -> dict:

@@ -164,6 +164,9 @@ def main():
     ap.add_argument("--cpu-particles", type=int, default=2048, help="oracle sample for cpu_baseline (0 = skip)")
     ap.add_argument("--ref-particles", type=int, default=1024)
     ap.add_argument("--no-peaks", action="store_true")
+    ap.add_argument("--ncell", type=int, default=0,
+                    help="cells per dimension instead of the workload's grid (0 = the workload's): a coarser grid "
+                         "changes cells less often, which separates the cost of cell fetches from the rest")
     args = ap.parse_args()
     cfg_idx = W.CONFIG_NAMES.index(args.workload)
     if args.impl == "reference":
@@ -187,7 +190,8 @@ def main():
 
     # ---- inputs: seeded, synthetic, resident in HBM before the timed region ---------------------
     n = args.particles if args.particles > 0 else None
-    cfg = W.config(cfg_idx, n=n, ensemble=rank)     # every rank traces its own ensemble (weak scaling)
+    ncell = [args.ncell] * 3 if args.ncell > 0 else None
+    cfg = W.config(cfg_idx, n=n, ncell=ncell, ensemble=rank)     # every rank traces its own ensemble (weak scaling)
     fd, pd = cfg["field"], cfg["params"]
     model = model_of(cfg)
     npart = cfg["x0"].shape[1]
@@ -333,7 +337,8 @@ def main():
     # ---- CPU oracle beside it (rank 0, N = 1 only) ---------------------------------------------------
     cpu = None
     if rank == 0 and world == 1 and args.cpu_particles > 0:
-        r = oracle_sample(W.config(cfg_idx, n=min(args.cpu_particles, npart)), args.window, args.cpu_particles)
+        r = oracle_sample(W.config(cfg_idx, n=min(args.cpu_particles, npart), ncell=ncell), args.window,
+                          args.cpu_particles)
         cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
                "seconds": r["seconds"]}
 

@@ -237,6 +237,9 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
       // (8 independent rows) is worked while the first batch of the shared half is in flight; the shared
       // half V comes slab by slab, each slab's two rows as ONE batch of four 16-byte loads issued as soon as
       // the previous batch has been consumed
+      const long long tl_h0 = TL_NOW();
+      (void)tl_h0;
+      if (tl_on) TL_ADD(6, tl_h0 - tl_wake);
       double v[8];
       lds_slab(strip_s + 64 * 3, v);
       double U;

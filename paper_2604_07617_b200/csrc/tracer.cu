@@ -81,8 +81,8 @@ struct SplitTraits {
   static constexpr size_t OFF_REQ = OFF_FV + (size_t)NQ * 32 * 8;    // int2   [32]: code, flat cell index
   static constexpr size_t OFF_POS = OFF_REQ + 32 * 8;                // float  [2][3][32]: last point, start point (cell units)
   static constexpr size_t OFF_GUESS = OFF_POS + 2 * 3 * 32 * 4;      // int    [32]: guessed cell of the next point
-  static constexpr size_t OFF_ERR = OFF_GUESS + 32 * 4;               // double [8][32]: known part of the error ratio
-  static constexpr size_t OFF_Y = OFF_ERR + 8 * 32 * 8;               // double [9][32]: state y at the start of the step, dt, stage partial sums
+  static constexpr size_t OFF_ERR = OFF_GUESS + 32 * 4;               // double [12][32]: known part of the error ratio; wave terms
+  static constexpr size_t OFF_Y = OFF_ERR + 12 * 32 * 8;               // double [9][32]: state y at the start of the step, dt, stage partial sums
   static constexpr size_t OFF_COLD = OFF_Y + 9 * 32 * 8;                   // per-lane bookkeeping: 5 x int64[32] + 8 x int32[32]
   static constexpr size_t OFF_TL = OFF_COLD + 5 * 256 + 8 * 128;     // int64 [4]: timestamps of the CATAPULT_TIMELINE build
   static constexpr size_t SMEM_BYTES = OFF_TL + 32 + 128;
@@ -459,10 +459,19 @@ __device__ __forceinline__ void publish_guess(unsigned char* smem, int lane, int
 
 template <int MODEL>
 __device__ __forceinline__ void eval_collect(const TraceConst& tc, unsigned char* smem, int lane, const double y[4],
-                                             double mu, const EvalGeo& g, double dy[4], double& modB,
-                                             double& level) {
+                                             double mu, EvalGeo& g, double dy[4], double& modB, double& level) {
   using ST = SplitTraits<MODEL>;
   const double* fvbuf = reinterpret_cast<const double*>(smem + ST::OFF_FV);
+  // The wave terms cross the barrier through shared memory: stores cannot move across a barrier, so the
+  // arithmetic that produces them stays in the overlap window (ptxas otherwise sinks it below the barrier, onto
+  // the critical path, to save the registers they would occupy across it).
+  double* wavebuf = reinterpret_cast<double*>(smem + ST::OFF_ERR) + 8 * 32 + lane;
+  if (MODEL == MODEL_BOOZER_SAW) {
+    wavebuf[0] = g.sn;
+    wavebuf[32] = g.cs;
+    wavebuf[64] = g.Phihat;
+    wavebuf[96] = g.dPhihat;
+  }
 #ifdef CATAPULT_TIMELINE
   volatile long long* tl = reinterpret_cast<volatile long long*>(smem + ST::OFF_TL);
   volatile unsigned long long* tl_acc = reinterpret_cast<volatile unsigned long long*>(smem + ST::OFF_TL + 32);
@@ -479,6 +488,12 @@ __device__ __forceinline__ void eval_collect(const TraceConst& tc, unsigned char
   double fv[ST::NQ];
 #pragma unroll
   for (int q = 0; q < ST::NQ; ++q) fv[q] = fvbuf[q * 32 + lane];
+  if (MODEL == MODEL_BOOZER_SAW) {
+    g.sn = wavebuf[0];
+    g.cs = wavebuf[32];
+    g.Phihat = wavebuf[64];
+    g.dPhihat = wavebuf[96];
+  }
   eval_physics<MODEL>(tc, y, mu, g, fv, dy, modB, level);
 }
 
@@ -672,14 +687,14 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
         dy[c] = ks[c * 32];  // k1 (first-same-as-last, or the start point's derivative)
         P[c * 32] = 0.0;
       }
-#pragma unroll 1
-      for (int st = 0; st < 6; ++st) {
+      EvalGeo g;
+      // one stage point: its state, the request, and everything that overlaps the contraction
+      auto stage_publish = [&](int st) {
         // stage state y + h sum_{j<=st} a[st][j] k_j (row 5 = b: the new state); the sum over j < st was
         // accumulated while the previous contraction ran, the newest derivative enters last
         const double ad = DP_A[st][st];
 #pragma unroll
         for (int c = 0; c < 4; ++c) ys[c] = fma(h, fma(ad, dy[c], P[c * 32]), ysm[c * 32]);
-        EvalGeo g;
         float pos[3];
         eval_publish<MODEL>(tc, smem, lane, stepping ? st : REQ_NONE, CTL_PLAIN, fma(DP_C[st], h, t), ys, g, pos);
         // ---- overlaps the contraction ----
@@ -717,10 +732,21 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
             errbuf[(4 + c) * 32] = fm::rcp(fma(tc.rtol, fma(ah, fabs(ks[c * 32]), fabs(ysm[c * 32])), sc));
           }
         }
+      };
+      // The loop is cut between the overlap window and the pick-up of the values, so that the critical part of a
+      // round (values -> physics -> next stage state -> locate -> request) is one straight-line block in which
+      // the compiler can interleave the short critical chain with the rest.
+      stage_publish(0);
+#pragma unroll 1
+      for (int st = 0; st < 5; ++st) {
         eval_collect<MODEL>(tc, smem, lane, ys, mu, g, dy, B_, level);
 #pragma unroll
         for (int c = 0; c < 4; ++c) ks[((st + 1) * 4 + c) * 32] = dy[c];
+        stage_publish(st + 1);
       }
+      eval_collect<MODEL>(tc, smem, lane, ys, mu, g, dy, B_, level);
+#pragma unroll
+      for (int c = 0; c < 4; ++c) ks[(6 * 4 + c) * 32] = dy[c];
       double r = 0.0, chk = 0.0;
 #pragma unroll
       for (int c = 0; c < 4; ++c) {

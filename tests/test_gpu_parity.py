@@ -383,6 +383,47 @@ def test_refill_queue_many_more_particles_than_threads(K, oracle):
     assert cnt[2] + cnt[3] == n
 
 
+@pytest.mark.parametrize("idx,n_full", [(4, 1_000_000), (3, 100_000), (2, 100_000)])
+def test_full_size_launch_sampled_against_oracle(K, oracle, idx, n_full):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (full grid, full particle count,
+    one 1e-5 s window through init + continue): a random sample of particles is traced one by one by the
+    oracle and compared within the method's global error; properties that hold at any size are checked on
+    all particles (statuses, stop times, counters, every index written exactly once)."""
+    cfg = W.config(idx, n=n_full)
+    fd, pd = cfg["field"], dict(cfg["params"], T=1e-5)
+    gf = K.catapult_field_build(fd)
+    st = K.catapult_trace_init(gf, pd, _dev(cfg["x0"]))
+    K.catapult_trace_continue(gf, pd, st)
+    torch.cuda.synchronize()
+    gs = st["status"].cpu().numpy()
+    gt = st["t"].cpu().numpy()
+    gx = st["x"].cpu().numpy()
+    na, nr = st["nacc"].cpu().numpy(), st["nrej"].cpu().numpy()
+    cnt = st["counters"].cpu().numpy()
+    assert gs.shape == (n_full,) and np.all((gs == 0) | (gs == 1))
+    assert np.all(gt[gs == 0] == pd["T"]) and np.all((gt[gs == 1] >= 0) & (gt[gs == 1] <= pd["T"]))
+    assert np.all(np.isfinite(gx))
+    assert cnt[0] == na.astype(np.int64).sum() and cnt[1] == nr.astype(np.int64).sum()
+    assert cnt[2] == np.sum(gs == 0) and cnt[3] <= np.sum(gs == 1) and cnt[6] >= 6 * (cnt[0] + cnt[1])
+    assert np.all(na[gs == 0] > 0)
+    pick = np.sort(np.random.default_rng(100 + idx).choice(n_full, size=48, replace=False))
+    of, op = oracle.Field(fd), oracle.make_params(pd)
+    x0s = np.ascontiguousarray(cfg["x0"][:, pick])
+    o = oracle.trace(of, op, x0s)
+    assert np.array_equal(gs[pick], o["status"])
+    ref = oracle.trace(of, oracle.make_params(dict(pd, rtol=1e-12, atol=1e-15)), x0s)
+    coord = fd["coord"]
+    nacc = o["nacc"].astype(float)
+    qg = _free_diff_over_tol(coord, gx[:, pick], ref["xf"], nacc, pd["rtol"])
+    qo = _free_diff_over_tol(coord, o["xf"], ref["xf"], nacc, pd["rtol"])
+    alive = o["status"] == 0
+    for comp in range(4):
+        assert qg[comp, alive].max() <= max(1.0, 3.0 * qo[comp, alive].max()), (comp, qg[comp].max(), qo[comp].max())
+    assert np.allclose(gt[pick][~alive], o["tstop"][~alive], rtol=0.05)
+    assert np.abs(na[pick].astype(int) - o["nacc"].astype(int)).max() <= 0.1 * o["nacc"].max() + 3
+    gf.destroy()
+
+
 def test_init_continue_equals_trace_and_windows(K, cases):
     c = cases[2]
     cfg = c["cfg"]

@@ -198,12 +198,13 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
   };
   auto issue_loads = [&](int c) {
     const double* src = table + ((long long)c * NQ + q) * 64;
+    // the eight vector loads first (they are the slower half: one request per 32 bytes), then the bulk copy
+#pragma unroll
+    for (int e = 0; e < 32; e += 4) ldg_f64x4(src + e, reg[e], reg[e + 1], reg[e + 2], reg[e + 3]);
     wait_strip();  // a wrong guess may still be landing in the strip: let it finish first
     mbar_expect_tx(mbar, 256);
     bulk_g2s(strip_s, src + 32, 256, mbar);
     pending = true;
-#pragma unroll
-    for (int e = 0; e < 32; e += 4) ldg_f64x4(src + e, reg[e], reg[e + 1], reg[e + 2], reg[e + 3]);
   };
 
   volatile long long* tl = reinterpret_cast<volatile long long*>(smem + ST::OFF_TL);

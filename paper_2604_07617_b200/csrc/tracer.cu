@@ -80,8 +80,8 @@ struct SplitTraits {
   static constexpr size_t OFF_FV = OFF_W + 3 * 32 * 8;               // double [NQ][32]
   static constexpr size_t OFF_REQ = OFF_FV + (size_t)NQ * 32 * 8;    // int2   [32]: code, flat cell index
   static constexpr size_t OFF_POS = OFF_REQ + 32 * 8;                // float  [2][3][32]: last point, start point (cell units)
-  static constexpr size_t OFF_GUESS = OFF_POS + 2 * 3 * 32 * 4;      // int    [32]: guessed cell of the next point
-  static constexpr size_t OFF_ERR = OFF_GUESS + 32 * 4;               // double [12][32]: known part of the error ratio; wave terms
+  static constexpr size_t OFF_GUESS = OFF_POS + 2 * 3 * 32 * 4;      // int    [2][32]: guessed cell of the next point, by round parity
+  static constexpr size_t OFF_ERR = OFF_GUESS + 2 * 32 * 4;               // double [12][32]: known part of the error ratio; wave terms
   static constexpr size_t OFF_Y = OFF_ERR + 12 * 32 * 8;               // double [9][32]: state y at the start of the step, dt, stage partial sums
   static constexpr size_t OFF_COLD = OFF_Y + 9 * 32 * 8;                   // per-lane bookkeeping: 5 x int64[32] + 8 x int32[32]
   static constexpr size_t OFF_TL = OFF_COLD + 5 * 256 + 8 * 128;     // int64 [4]: timestamps of the CATAPULT_TIMELINE build
@@ -219,7 +219,7 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
     if (tl_on) { TL_ADD(9, tl_wake - tl_t0); TL_ADD(5, tl_wake - tl[0]); }
     const long long rq_raw = *reinterpret_cast<const volatile long long*>(reqbuf + lane);  // one 8-byte load
     const int2 rq = make_int2((int)rq_raw, (int)(rq_raw >> 32));
-    const int ctl = rq.x >> 3;                                  // block-uniform
+    const int ctl = (rq.x >> 3) & 7;                            // block-uniform
     if (ctl == CTL_QUIT) break;
     const int code = (rq.x & 7) == 7 ? REQ_NONE : (rq.x & 7);
     if (code >= 0) {
@@ -282,7 +282,7 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
     // fetching that cell if it is not the one held.  A wrong guess costs what every cell change cost before
     // (a blocking fetch next round); a right one hides the fetch entirely.
     bar_sync(3, NT);
-    int target = guessbuf[lane];
+    int target = guessbuf[((rq.x >> 6) & 1) * 32 + lane];  // double-buffered by round parity
     if (code < 0 || target < 0) target = cached;
     if (target != cached) {
 #ifdef CATAPULT_PF_STATS
@@ -421,7 +421,7 @@ __device__ __forceinline__ void stage_partial(const double* ks, double* P) {  //
 // anything that does not need field values (it overlaps the contraction).  All 32 lanes must call both.
 template <int MODEL>
 __device__ __forceinline__ void eval_publish(const TraceConst& tc, unsigned char* smem, int lane, int code, int ctl,
-                                             double t, const double y[4], EvalGeo& g, float pos[3]) {
+                                             int& rpar, double t, const double y[4], EvalGeo& g, float pos[3]) {
   using ST = SplitTraits<MODEL>;
   double* wbuf = reinterpret_cast<double*>(smem + ST::OFF_W);
   int2* reqbuf = reinterpret_cast<int2*>(smem + ST::OFF_REQ);
@@ -433,7 +433,8 @@ __device__ __forceinline__ void eval_publish(const TraceConst& tc, unsigned char
   wbuf[lane] = w[0];
   wbuf[32 + lane] = w[1];
   wbuf[64 + lane] = w[2];
-  reqbuf[lane] = make_int2((code < 0 ? 7 : code) | (ctl << 3), cell);  // one word: what to do + what follows
+  rpar ^= 1;  // round parity: selects the guess buffer of this round
+  reqbuf[lane] = make_int2((code < 0 ? 7 : code) | (ctl << 3) | (rpar << 6), cell);  // one word: what to do + what follows
 #pragma unroll
   for (int d = 0; d < 3; ++d) posbuf[d * 32 + lane] = pos[d];
   __syncwarp();
@@ -451,9 +452,9 @@ __device__ __forceinline__ void eval_publish(const TraceConst& tc, unsigned char
 
 // the scalar warp's guess of the next evaluation point's cell (-1: none), handed over through barrier 3
 template <int MODEL>
-__device__ __forceinline__ void publish_guess(unsigned char* smem, int lane, int target) {
+__device__ __forceinline__ void publish_guess(unsigned char* smem, int lane, int rpar, int target) {
   using ST = SplitTraits<MODEL>;
-  reinterpret_cast<volatile int*>(smem + ST::OFF_GUESS)[lane] = target;
+  reinterpret_cast<volatile int*>(smem + ST::OFF_GUESS)[rpar * 32 + lane] = target;
   __syncwarp();
   bar_arrive(3, ST::NT);
 }
@@ -499,18 +500,19 @@ __device__ __forceinline__ void eval_collect(const TraceConst& tc, unsigned char
 }
 
 template <int MODEL>
-__device__ __forceinline__ void eval_round(const TraceConst& tc, unsigned char* smem, int lane, int code, double t,
-                                           const double y[4], double mu, double dy[4], double& modB, double& level) {
+__device__ __forceinline__ void eval_round(const TraceConst& tc, unsigned char* smem, int lane, int code, int& rpar,
+                                           double t, const double y[4], double mu, double dy[4], double& modB,
+                                           double& level) {
   using ST = SplitTraits<MODEL>;
   EvalGeo g;
   float pos[3];
-  eval_publish<MODEL>(tc, smem, lane, code, CTL_PLAIN, t, y, g, pos);
+  eval_publish<MODEL>(tc, smem, lane, code, CTL_PLAIN, rpar, t, y, g, pos);
   if (code >= 0) {  // a start point: the next attempted step is extrapolated from here
     float* basebuf = reinterpret_cast<float*>(smem + ST::OFF_POS) + 96;
 #pragma unroll
     for (int d = 0; d < 3; ++d) basebuf[d * 32 + lane] = pos[d];
   }
-  publish_guess<MODEL>(smem, lane, -1);
+  publish_guess<MODEL>(smem, lane, rpar, -1);
   eval_collect<MODEL>(tc, smem, lane, y, mu, g, dy, modB, level);
 }
 
@@ -566,6 +568,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
 #pragma unroll
   for (int j = 0; j < 4; ++j) c_fin[j * 32] = 0;
   bool active = false, exhausted = false;
+  int rpar = 0;  // parity of the evaluation round (the guess buffer is double-buffered by it)
 
   for (;;) {
     // ---- refill: lanes without a particle pull the next index (one atomic per warp) ------------------
@@ -606,7 +609,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
     if (__any_sync(FULL, fresh)) {
       // the start point's field values give mu and k1
       double dy0[4], B, level;
-      eval_round<MODEL>(tc, smem, lane, fresh ? REQ_START : REQ_NONE, t, y, 0.0, dy0, B, level);
+      eval_round<MODEL>(tc, smem, lane, fresh ? REQ_START : REQ_NONE, rpar, t, y, 0.0, dy0, B, level);
       if (fresh) {
         ++c_eval;
         if (MODE != MODE_STEP_ONCE && a.resume) {
@@ -639,7 +642,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
       // k1 with the particle's own mu: the field values are those of the round above; only the physics
       // is redone (mu enters linearly; the geometry is recomputed from y, cheap and rare)
       if (__any_sync(FULL, fresh && active)) {
-        eval_round<MODEL>(tc, smem, lane, (fresh && active) ? REQ_START : REQ_NONE, t, y, mu, dy0, B, level);
+        eval_round<MODEL>(tc, smem, lane, (fresh && active) ? REQ_START : REQ_NONE, rpar, t, y, mu, dy0, B, level);
         if (fresh && active) {
           ++c_eval;
 #pragma unroll
@@ -697,7 +700,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
 #pragma unroll
         for (int c = 0; c < 4; ++c) ys[c] = fma(h, fma(ad, dy[c], P[c * 32]), ysm[c * 32]);
         float pos[3];
-        eval_publish<MODEL>(tc, smem, lane, stepping ? st : REQ_NONE, CTL_PLAIN, fma(DP_C[st], h, t), ys, g, pos);
+        eval_publish<MODEL>(tc, smem, lane, stepping ? st : REQ_NONE, CTL_PLAIN, rpar, fma(DP_C[st], h, t), ys, g, pos);
         // ---- overlaps the contraction ----
         if (st < 5 || MODE == MODE_STEP_ONCE) {
           // the next point's cell, guessed by straight-line extrapolation from the step's start point (fp32,
@@ -708,7 +711,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
             const float base[3] = {basebuf[lane], basebuf[32 + lane], basebuf[64 + lane]};
             target = guess_cell<MODEL>(tc.f, pos, base, next_point_ratio(st));
           }
-          publish_guess<MODEL>(smem, lane, target);
+          publish_guess<MODEL>(smem, lane, rpar, target);
         }
         if (st < 5) {
           switch (st) {  // all the loads of a row first, then its sums (j ascending, as everywhere)
@@ -784,7 +787,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
             for (int d = 0; d < 3; ++d) posbuf[96 + d * 32 + lane] = pe[d];
           }
         }
-        publish_guess<MODEL>(smem, lane, target);
+        publish_guess<MODEL>(smem, lane, rpar, target);
       }
       if (stepping) {
         c_eval += 6;

@@ -123,6 +123,20 @@ def oracle_sample(cfg, window: float, nsample: int, nthreads: int = 0) -> dict:
                 sample=f"first {x0.shape[1]} particles of {cfg['name']} over [0, {window:g}] s")
 
 
+def reduce_over_ranks(time_value: float, counts, world: int, device):
+    """Whole-job figures of a weak-scaling run: the time is the MAX over ranks, every count the SUM over ranks
+    (each rank traces its own ensemble; there is no data-path collective, only this).  Returns (time, [counts])."""
+    if world <= 1:
+        return float(time_value), [float(c) for c in counts]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(time_value)], dtype=torch.float64, device=device)
+    c = torch.tensor([float(v) for v in counts], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t.item()), [float(v) for v in c.tolist()]
+
+
 def run_reference(args, cfg_idx: int):
     """--impl reference: the oracle on the host cores (rank 0 only under torchrun)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -252,15 +266,7 @@ def main():
     for f in fields:
         f.destroy()
     cnt = (state["counters"] - cnt0).cpu().numpy().astype(np.float64)
-    tvals = torch.tensor([ms, cnt[0], cnt[0] + cnt[1], cnt[6]], dtype=torch.float64, device="cuda")
-    if world > 1:
-        tmax = tvals.clone()
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = tvals.clone()
-        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        ms_all, acc_all, att_all, evals_all = tmax[0].item(), tsum[1].item(), tsum[2].item(), tsum[3].item()
-    else:
-        ms_all, acc_all, att_all, evals_all = ms, cnt[0], cnt[0] + cnt[1], cnt[6]
+    ms_all, (acc_all, att_all, evals_all) = reduce_over_ranks(ms, [cnt[0], cnt[0] + cnt[1], cnt[6]], world, "cuda")
     value = acc_all / (ms_all * 1e-3)
     loss_fraction = float(est[0].item())
     alive = int((state["status"] == 0).sum().item())
@@ -322,13 +328,7 @@ def main():
         torch.cuda.synchronize()
         dt_e2e = time.perf_counter() - t0
         acc_e2e = float(host["counters"][0] - c0[0])
-        tv = torch.tensor([dt_e2e, acc_e2e], dtype=torch.float64, device="cuda")
-        if world > 1:
-            tm = tv.clone()
-            dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-            ts = tv.clone()
-            dist.all_reduce(ts, op=dist.ReduceOp.SUM)
-            dt_e2e, acc_e2e = tm[0].item(), ts[1].item()
+        dt_e2e, (acc_e2e,) = reduce_over_ranks(dt_e2e, [acc_e2e], world, "cuda")
         e2e = {"value": acc_e2e / dt_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                "steps": args.e2e_steps, "ms_per_step": 1e3 * dt_e2e / args.e2e_steps,
                "api": "catapult_trace_continue_host (pinned host buffers)"}

@@ -368,12 +368,12 @@ def main():
 
 def _ncu_traffic(model: str, evals_per_launch: float):
     """DRAM bytes of one trace launch: `dram__bytes_read.sum + dram__bytes_write.sum` per right-hand-side
-    evaluation of the committed `ncu --set full` capture (profiles/r1_traffic_v4.md; cfg4 recipe) times the
+    evaluation of the committed `ncu --set full` capture (profiles/r1_traffic_v5.md; cfg4 recipe) times the
     evaluations of one timed launch.  None for the models that were not captured."""
     if model != "boozer_saw":
         return None
     try:
-        for line in open(os.path.join(ROOT, "profiles", "r1_traffic_v4.csv")):
+        for line in open(os.path.join(ROOT, "profiles", "r1_traffic_v5.csv")):
             f = line.strip().split(",")
             if f[0] == "dram_bytes_per_rhs_eval":
                 return float(f[1]) * evals_per_launch

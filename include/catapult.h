@@ -88,9 +88,13 @@ typedef struct {
 /* ---- field tables ------------------------------------------------
  * catapult_field_build: d_nodes holds the unique nodes [nquant][3*ncell0+1][3*ncell1+1][3*ncell2+1]
  * (last index fastest).  A device kernel gathers, for every cell, the 4x4x4 nodal block of every
- * quantity (shared faces duplicated) into the cell-major table
- * [cell][quantity][64] (cell = (i0*ncell1+i1)*ncell2+i2, node = (a*4+b)*4+c): one cell's
- * coefficients of one quantity are four 128-byte lines.  *out owns the table; d_nodes may be
+ * quantity (shared faces duplicated) and stores the cell's tricubic -- the SAME
+ * polynomial as the Lagrange interpolant of those 64 nodes -- as its 64 coefficients
+ * in the centred monomials w0^i w1^j w2^k, w = 2u-1 (basis change in double-double arithmetic), in the
+ * cell-major table [cell][quantity][64] (cell = (i0*ncell1+i1)*ncell2+i2; inside a 512-byte block the
+ * rows j = 0,1 first, then j = 2,3: an internal order).  One cell's
+ * coefficients of one quantity are four 128-byte lines.  catapult_field_export_rows recovers the
+ * nodal values in the paper's own row layout.  *out owns the table; d_nodes may be
  * freed once the stream has run.  Errors: EINVAL (NULL, ncell<1, nquant mismatch, hi<=lo),
  * EUNSUPPORTED (Boozer I0 != 0), ENOMEM, ECUDA. */
 catapult_status catapult_field_build(const catapult_field_desc *desc, const double *d_nodes,

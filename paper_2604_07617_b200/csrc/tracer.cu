@@ -222,6 +222,8 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
     const int ctl = (rq.x >> 3) & 7;                            // block-uniform
     if (ctl == CTL_QUIT) break;
     const int code = (rq.x & 7) == 7 ? REQ_NONE : (rq.x & 7);
+    // the local coordinates are loaded with the request, not after it has been looked at (one latency, not two)
+    const double w0 = wbuf[lane], w1 = wbuf[32 + lane], w2 = wbuf[64 + lane];
     if (code >= 0) {
       const int c = rq.y;
       if (c != cached) {  // the guess missed (or there was none): one memory latency, paid by the whole block
@@ -233,7 +235,6 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
 #endif
       }
       wait_strip();
-      const double w0 = wbuf[lane], w1 = wbuf[32 + lane], w2 = wbuf[64 + lane];
       // horner64 (gc_device.cuh), same operations in the same order, scheduled by hand: the register half U
       // (8 independent rows) is worked while the first batch of the shared half is in flight; the shared
       // half V comes slab by slab, each slab's two rows as ONE batch of four 16-byte loads issued as soon as

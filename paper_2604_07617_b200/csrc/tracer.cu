@@ -11,11 +11,16 @@
 //     memory), re-fetched from the cell-major table only when the slot's cell changes.  Per evaluation it
 //     reads the slot's (cell, w) from shared memory, evaluates the 64-coefficient polynomial by nested
 //     Horner (63 FMA, gc_device.cuh) and writes one value back.
-// The two sides meet through two named barriers per evaluation (bar.arrive / bar.sync producer-consumer
-// pairs): the scalar warp publishes (cell, w) and -- while the contraction warps work -- evaluates
-// everything that does not need field values (the wave's exp / sincos); then it picks up the NQ values.
-// The seven stage derivatives live in shared memory, so the stage loop is rolled (one copy of the
-// right-hand side in the instruction stream).
+// The two sides meet through named barriers (bar.arrive / bar.sync producer-consumer pairs): 1 = request
+// published, 2 = values ready, 3 = guess published.  While the contraction warps work the scalar warp evaluates
+// everything that does not need field values (the wave's exp / sincos, the next stage's partial sums, the
+// known part of the error ratio) and GUESSES THE NEXT POINT'S CELL (fp32, straight-line extrapolation along
+// the attempted step; at the end of an attempt from the accept/reject decision and the controller's new step
+// length).  A contraction lane starts fetching the guessed cell as soon as it is done with the current point
+// (eight 256-bit loads for the register half, one bulk asynchronous copy for the shared half), so the fetch
+// overlaps the scalar warp's work; a wrong guess only costs a blocking fetch.  The seven stage derivatives,
+// the step's start state and the per-particle bookkeeping live in shared memory, so the stage loop is rolled
+// (one copy of the right-hand side in the instruction stream) and nothing spills.
 #include <cstdlib>
 
 #include "gc_device.cuh"
@@ -36,15 +41,6 @@ __device__ unsigned long long g_blk[8];  // debugging aid: blocking fetches by r
 extern "C" int catapult_debug_blocking(unsigned long long* out8) {
   return cudaMemcpyFromSymbol(out8, g_blk, sizeof(g_blk)) != cudaSuccess;
 }
-#endif
-#ifdef CATAPULT_TIMELINE
-// debugging aid (not part of the product build): cycle counts of the phases of a round, summed over rounds
-__device__ unsigned long long g_tl[16];
-#define TL_NOW() clock64()
-#define TL_ADD(slot, v) (tl_acc[slot] += (unsigned long long)(v))
-#else
-#define TL_NOW() 0LL
-#define TL_ADD(slot, v) ((void)0)
 #endif
 
 // Dormand-Prince 5(4) tableau for the rolled stage loop (row i = coefficients of the state fed to stage
@@ -84,8 +80,7 @@ struct SplitTraits {
   static constexpr size_t OFF_ERR = OFF_GUESS + 2 * 32 * 4;               // double [12][32]: known part of the error ratio; wave terms
   static constexpr size_t OFF_Y = OFF_ERR + 12 * 32 * 8;               // double [9][32]: state y at the start of the step, dt, stage partial sums
   static constexpr size_t OFF_COLD = OFF_Y + 9 * 32 * 8;                   // per-lane bookkeeping: 5 x int64[32] + 8 x int32[32]
-  static constexpr size_t OFF_TL = OFF_COLD + 5 * 256 + 8 * 128;     // int64 [4]: timestamps of the CATAPULT_TIMELINE build
-  static constexpr size_t SMEM_BYTES = OFF_TL + 32 + 128;
+  static constexpr size_t SMEM_BYTES = OFF_COLD + 5 * 256 + 8 * 128;
 };
 
 // Request of a slot: one word (what to evaluate: a stage point 0..5 of an attempted step, a start point, or
@@ -206,17 +201,8 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
     bulk_g2s(strip_s, src + 32, 256, mbar);
     pending = true;
   };
-
-  volatile long long* tl = reinterpret_cast<volatile long long*>(smem + ST::OFF_TL);
-  volatile unsigned long long* tl_acc = reinterpret_cast<volatile unsigned long long*>(smem + ST::OFF_TL + 32);
-  (void)tl_acc;
-  const bool tl_on = (q == 0 && lane == 0);
-  long long tl_t0 = TL_NOW();
   for (;;) {
     bar_sync(1, NT);
-    const long long tl_wake = TL_NOW();
-    (void)tl_wake;
-    if (tl_on) { TL_ADD(9, tl_wake - tl_t0); TL_ADD(5, tl_wake - tl[0]); }
     const long long rq_raw = *reinterpret_cast<const volatile long long*>(reqbuf + lane);  // one 8-byte load
     const int2 rq = make_int2((int)rq_raw, (int)(rq_raw >> 32));
     const int ctl = (rq.x >> 3) & 7;                            // block-uniform
@@ -239,9 +225,6 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
       // (8 independent rows) is worked while the first batch of the shared half is in flight; the shared
       // half V comes slab by slab, each slab's two rows as ONE batch of four 16-byte loads issued as soon as
       // the previous batch has been consumed
-      const long long tl_h0 = TL_NOW();
-      (void)tl_h0;
-      if (tl_on) TL_ADD(6, tl_h0 - tl_wake);
       double v[8];
       lds_slab(strip_s + 64 * 3, v);
       double U;
@@ -272,11 +255,8 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
       }
       const double total = fma(V, w1 * w1, U);
       fvbuf[q * 32 + lane] = total;
-      if (tl_on) TL_ADD(7, TL_NOW() - tl_h0);
     }
     __syncwarp();
-    const long long tl_a2 = TL_NOW();
-    if (tl_on) tl[1] = tl_a2;
     bar_arrive(2, NT);
     // ---- while the scalar warp works: it publishes its guess of the NEXT point's cell (barrier 3: in its
     // overlap window inside an attempted step; right after the accept/reject decision at its end); start
@@ -292,8 +272,6 @@ __device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned c
       issue_loads(target);
       cached = target;
     }
-    tl_t0 = TL_NOW();
-    if (tl_on) TL_ADD(8, tl_t0 - tl_a2);
   }
 #ifdef CATAPULT_PF_STATS
   if (counters && q == 0) {  // debugging aid: blocking / guessed fetches of quantity 0 in the two spare status counters
@@ -439,14 +417,6 @@ __device__ __forceinline__ void eval_publish(const TraceConst& tc, unsigned char
 #pragma unroll
   for (int d = 0; d < 3; ++d) posbuf[d * 32 + lane] = pos[d];
   __syncwarp();
-#ifdef CATAPULT_TIMELINE
-  {
-    volatile long long* tl = reinterpret_cast<volatile long long*>(smem + ST::OFF_TL);
-    volatile unsigned long long* tl_acc = reinterpret_cast<volatile unsigned long long*>(smem + ST::OFF_TL + 32);
-    const long long now = TL_NOW();
-    if (lane == 0) { TL_ADD(0, 1); TL_ADD(1, now - tl[2]); tl[0] = now; }
-  }
-#endif
   bar_arrive(1, ST::NT);
   eval_wave<MODEL>(tc, t, y, g);
 }
@@ -475,19 +445,7 @@ __device__ __forceinline__ void eval_collect(const TraceConst& tc, unsigned char
     wavebuf[64] = g.Phihat;
     wavebuf[96] = g.dPhihat;
   }
-#ifdef CATAPULT_TIMELINE
-  volatile long long* tl = reinterpret_cast<volatile long long*>(smem + ST::OFF_TL);
-  volatile unsigned long long* tl_acc = reinterpret_cast<volatile unsigned long long*>(smem + ST::OFF_TL + 32);
-  const long long tl_b = TL_NOW();
-  if (lane == 0) TL_ADD(2, tl_b - tl[0]);
-#endif
   bar_sync(2, ST::NT);
-#ifdef CATAPULT_TIMELINE
-  {
-    const long long now = TL_NOW();
-    if (lane == 0) { TL_ADD(3, now - tl_b); TL_ADD(4, now - tl[1]); tl[2] = now; }
-  }
-#endif
   double fv[ST::NQ];
 #pragma unroll
   for (int q = 0; q < ST::NQ; ++q) fv[q] = fvbuf[q * 32 + lane];
@@ -524,18 +482,8 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
   extern __shared__ __align__(16) unsigned char smem[];
   const int lane = threadIdx.x & 31;
   const int warp = threadIdx.x >> 5;
-#ifdef CATAPULT_TIMELINE
-  if (threadIdx.x < 16) reinterpret_cast<unsigned long long*>(smem + ST::OFF_TL + 32)[threadIdx.x] = 0;
-  if (threadIdx.x < 4) reinterpret_cast<long long*>(smem + ST::OFF_TL)[threadIdx.x] = clock64();
-  __syncthreads();
-#endif
   if (warp < ST::NQ) {
     contraction_warp<MODEL>(tc.f, smem, warp, lane, a.counters);
-#ifdef CATAPULT_TIMELINE
-    if (warp == 0 && lane == 0)
-      for (int j = 5; j < 10; ++j)
-        atomicAdd(&g_tl[j], reinterpret_cast<unsigned long long*>(smem + ST::OFF_TL + 32)[j]);
-#endif
     return;
   }
 
@@ -856,10 +804,6 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
     bar_arrive(1, ST::NT);
   }
 
-#ifdef CATAPULT_TIMELINE
-  if (lane == 0)
-    for (int j = 0; j < 5; ++j) atomicAdd(&g_tl[j], reinterpret_cast<unsigned long long*>(smem + ST::OFF_TL + 32)[j]);
-#endif
   // ---- statistics: one atomic per warp per counter -----------------------------------------------------
   if (a.counters) {
     unsigned long long v[7] = {c_acc, c_rej, c_fin[0], c_fin[32], c_fin[64], c_fin[96], c_eval};
@@ -929,16 +873,6 @@ catapult_status launch_trace(const TraceConst& tc, const TraceArgs& a, int model
   }
 }
 
-#ifdef CATAPULT_TIMELINE
-extern "C" int catapult_debug_timeline(unsigned long long* out16, int reset) {
-  if (out16 && cudaMemcpyFromSymbol(out16, g_tl, sizeof(g_tl)) != cudaSuccess) return 1;
-  if (reset) {
-    unsigned long long z[16] = {0};
-    if (cudaMemcpyToSymbol(g_tl, z, sizeof(z)) != cudaSuccess) return 1;
-  }
-  return 0;
-}
-#endif
 
 catapult_status trace_launch_shape(int model, int64_t n, int* blocks, int* threads) {
   switch (model) {

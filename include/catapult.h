@@ -15,8 +15,11 @@
  *   - Every call returns a catapult_status; no exception crosses the boundary;
  *     catapult_last_error() returns a thread-local message for the last failing call.
  *   - Calls validate their arguments synchronously, enqueue work on `stream` and do not
- *     synchronise, except the *_host variants and catapult_estimate with a non-NULL h_out, which
- *     return after their results are in host memory.
+ *     synchronise (device memory they need is allocated and freed stream-ordered), except: the
+ *     *_host variants and catapult_estimate with a non-NULL h_out, which return after their
+ *     results are in host memory, and catapult_field_destroy / catapult_release_host_cache,
+ *     which free device memory (cudaFree).  A field may be used on any stream: every call that
+ *     reads its tables is ordered after the build by an event the build recorded.
  *   - There is no CPU fallback anywhere: without a CUDA device every compute call fails with
  *     CATAPULT_ECUDA.
  *   - Particle arrays are structure-of-arrays: x[4][n] means component c of particle i at
@@ -50,6 +53,20 @@ typedef enum {
 #define CATAPULT_NQUANT_BOOZER 4
 #define CATAPULT_NQUANT_CYL 7
 
+/* semantic tags of the columns (catapult_field_desc.quant).  All sixteen entries zero = the canonical
+   order above; otherwise quant[0..nquant) must spell out that same order (other orders: EUNSUPPORTED) */
+#define CATAPULT_Q_MODB 1
+#define CATAPULT_Q_DMODB_DS 2
+#define CATAPULT_Q_DMODB_DTHETA 3
+#define CATAPULT_Q_DMODB_DZETA 4
+#define CATAPULT_Q_B_R 5
+#define CATAPULT_Q_B_PHI 6
+#define CATAPULT_Q_B_Z 7
+#define CATAPULT_Q_DMODB_DR 8
+#define CATAPULT_Q_DMODB_DPHI_OVER_R 9
+#define CATAPULT_Q_DMODB_DZ 10
+#define CATAPULT_Q_PSI_LEVEL 11
+
 /* particle status */
 #define CATAPULT_ST_REACHED_T 0
 #define CATAPULT_ST_LOST 1      /* s >= 1 (Boozer) or psi >= psi_edge (Cartesian) */
@@ -62,12 +79,17 @@ typedef struct {
                        unique nodes per dimension = 3*ncell+1 */
   int32_t nfp;      /* field periods: the last grid dimension spans [lo, lo + 2pi/nfp) */
   int32_t nquant;   /* m, must equal CATAPULT_NQUANT_* of `coord` */
+  int32_t quant[16]; /* CATAPULT_Q_* tag of every column, or all zero (= the canonical order of `coord`) */
   double lo[3], hi[3]; /* Boozer: [0,1],[0,2pi],[0,2pi/nfp]; cyl: [Rmin,Rmax],[Zmin,Zmax],[0,2pi/nfp].
                           theta, zeta and phi are periodic with period hi-lo; s, R, Z extrapolate
                           with the nearest cell's cubic outside [lo,hi] */
   double G0, I0;       /* Boozer covariant components, constants (vacuum: I0 must be 0) */
   double iota0, iota1; /* rotational transform iota(s) = iota0 + iota1*s */
   double psi0;         /* Boozer: toroidal flux/(2pi) at s=1; cyl: psi_edge (loss level) */
+  /* Boozer 1-D profiles on the s-nodes (iota "represented on a regular interpolant grid"):
+     DEVICE pointers to 3*ncell[0]+1 doubles each, NULL = use the scalars / the linear law above.
+     Non-NULL is valid but not built yet (EUNSUPPORTED): every BASELINE config uses the scalars. */
+  const double *G_nodes, *I_nodes, *iota_nodes;
 } catapult_field_desc;
 
 typedef struct catapult_field catapult_field; /* opaque; owns the per-cell coefficient tables */
@@ -78,7 +100,8 @@ typedef struct {
   double rtol, atol;           /* Eq. 4; atol is multiplied by v_total for vpar
                                                                                    */
   double dt0, dtmax;           /* initial / maximum step; <= 0 selects the defaults of DESIGN.md S3 */
-  int64_t max_steps;           /* attempts per particle per call; 0 = unlimited                 */
+  int64_t max_steps;           /* attempts per particle PER CALL (every catapult_trace_continue
+                                  window starts a new count); 0 = unlimited                     */
   int32_t max_consecutive_rejects; /* 0 = 500                                                   */
   int32_t saw_on;              /* 1: shear Alfven wave, Boozer only              */
   int32_t saw_m, saw_n;        /* Phi = Phi0 exp(-(s-s0)^2/w2) sin(m theta - n zeta + omega t)  */
@@ -90,13 +113,14 @@ typedef struct {
  * (last index fastest).  A device kernel gathers, for every cell, the 4x4x4 nodal block of every
  * quantity (shared faces duplicated) and stores the cell's tricubic -- the SAME
  * polynomial as the Lagrange interpolant of those 64 nodes -- as its 64 coefficients
- * in the centred monomials w0^i w1^j w2^k, w = 2u-1 (basis change in double-double arithmetic), in the
+ * in the centred monomials w0^p0 w1^p1 w2^p2, w = 2u-1 (basis change in double-double arithmetic), in the
  * cell-major table [cell][quantity][64] (cell = (i0*ncell1+i1)*ncell2+i2; inside a 512-byte block the
- * rows j = 0,1 first, then j = 2,3: an internal order).  One cell's
- * coefficients of one quantity are four 128-byte lines.  catapult_field_export_rows recovers the
- * nodal values in the paper's own row layout.  *out owns the table; d_nodes may be
- * freed once the stream has run.  Errors: EINVAL (NULL, ncell<1, nquant mismatch, hi<=lo),
- * EUNSUPPORTED (Boozer I0 != 0), ENOMEM, ECUDA. */
+ * coefficients are ordered by the power of theta (phi) first, then s (R), then zeta (Z): an internal
+ * order).  One cell's coefficients of one quantity are four 128-byte lines.
+ * catapult_field_export_rows recovers the nodal values in the paper's own row layout.  *out owns the
+ * table (allocated stream-ordered on `stream`); d_nodes may be freed once the stream has run.
+ * Errors: EINVAL (NULL, ncell<1 or more than 2^31-1 cells, nquant mismatch, hi<=lo), EUNSUPPORTED
+ * (Boozer I0 != 0, tabulated profiles, non-canonical column order), ENOMEM, ECUDA. */
 catapult_status catapult_field_build(const catapult_field_desc *desc, const double *d_nodes,
                                      void *stream, catapult_field **out);
 /* same with HOST nodes: copies them to the device, builds, synchronises, frees the staging copy */
@@ -120,9 +144,12 @@ catapult_status catapult_field_export_rows(const catapult_field *f, double *d_ou
  * coordinates (Boozer theta in (-pi,pi], zeta unreduced), d_tstop[n] = min(tau,T),
  * d_status[n] = CATAPULT_ST_*; d_nacc/d_nrej[n] (may be NULL) = accepted / rejected attempts.
  * A particle already outside at t=0 is returned unchanged with status LOST and t_stop = 0.
- * d_counters (may be NULL): 8 uint64 accumulated (atomically added) by the kernel:
+ * d_counters (may be NULL): CATAPULT_NCOUNTERS uint64 accumulated (atomically added) by the kernel:
  *   [0] accepted steps, [1] rejected attempts, [2] particles finished at T, [3] lost,
- *   [4] stalled, [5] max_steps, [6] right-hand-side evaluations, [7] cell-table (re)loads. */
+ *   [4] stalled, [5] max_steps, [6] right-hand-side evaluations, [7] cell fetches from the table,
+ *   [8] of which blocking (the cell was not the one fetched ahead), [9] evaluation rounds of the
+ *   32-slot blocks ([6] / (32 [9]) = fraction of slots doing useful work). */
+#define CATAPULT_NCOUNTERS 10
 catapult_status catapult_trace(const catapult_field *f, const catapult_trace_params *p, int64_t n,
                                const double *d_x0, double *d_xf, double *d_tstop,
                                int32_t *d_status, uint32_t *d_nacc, uint32_t *d_nrej,
@@ -140,7 +167,10 @@ catapult_status catapult_trace_continue(const catapult_field *f, const catapult_
                                         double *d_mu, int32_t *d_status, uint32_t *d_nacc,
                                         uint32_t *d_nrej, uint64_t *d_counters, void *stream);
 /* HOST-buffer form of catapult_trace: copies h_x0 to the device, traces, copies the results back
-   and synchronises.  h_nacc/h_nrej/h_counters may be NULL. */
+   and synchronises.  h_nacc/h_nrej/h_counters may be NULL.  The *_host calls keep one device staging
+   slab and one non-blocking stream per host thread between calls (grown on demand);
+   catapult_release_host_cache frees the calling thread's.  Pinned host buffers make the copies
+   asynchronous with respect to the host. */
 catapult_status catapult_trace_host(const catapult_field *f, const catapult_trace_params *p,
                                     int64_t n, const double *h_x0, double *h_xf, double *h_tstop,
                                     int32_t *h_status, uint32_t *h_nacc, uint32_t *h_nrej,
@@ -151,6 +181,7 @@ catapult_status catapult_trace_continue_host(const catapult_field *f, const cata
                                              int64_t n, double *h_x, double *h_t, double *h_dt,
                                              double *h_mu, int32_t *h_status, uint32_t *h_nacc,
                                              uint32_t *h_nrej, uint64_t *h_counters);
+catapult_status catapult_release_host_cache(void);
 /* test hook: scripted replay.  Every particle starts at t = 0 from d_x0[4][n] and takes the step sizes
    d_h[nsteps][n] (step-major) one after the other, each step ACCEPTED whatever its error ratio (the
    controller is bypassed); a particle stops at its first h <= 0, after nsteps steps, or when an end
@@ -180,31 +211,9 @@ catapult_status catapult_estimate(int32_t g_kind, int64_t n, const int32_t *d_st
                                   const double *d_tstop, const double *d_g_user, double *d_out,
                                   double *h_out, void *stream);
 
-/* ---- measurement hooks (roofline denominators) ---------------------
- * catapult_measure_fp64_peak: runs a register-only DFMA kernel on every SM and returns the
- * sustained double-precision rate in FLOP/s (2 per DFMA).
- * catapult_measure_l2_bandwidth: repeatedly reads a `bytes`-sized device buffer (choose it below
- * the L2 size) with 16-byte loads and returns bytes/s.  Both synchronise. */
-catapult_status catapult_measure_fp64_peak(double *flops_per_s);
-catapult_status catapult_measure_l2_bandwidth(size_t bytes, double *bytes_per_s);
 /* launch geometry the tracer uses on the current device: persistent blocks and threads per block */
 catapult_status catapult_trace_launch_shape(const catapult_field *f, const catapult_trace_params *p,
                                             int32_t *blocks, int32_t *threads);
-
-/* test hook: the device-side fp64 elementary functions the tracer's scalar path uses (csrc/gc_math.cuh)
-   evaluated elementwise on d_a[n] (and d_b[n] where a second argument exists):
-     ATAN2: out0 = atan2(a, b);  SINCOS: out0 = sin(a), out1 = cos(a);  EXP: out0 = exp(a);
-     SQRT_RSQRT: out0 = sqrt(a), out1 = 1/sqrt(a);  RCP: out0 = 1/a;
-     POW_NEG_INV: out0 = a^(-1/5), out1 = a^(-1/3) (the step-size controller's powers).
-   d_b and d_out1 may be NULL where unused. */
-#define CATAPULT_FN_ATAN2 0
-#define CATAPULT_FN_SINCOS 1
-#define CATAPULT_FN_EXP 2
-#define CATAPULT_FN_SQRT_RSQRT 3
-#define CATAPULT_FN_RCP 4
-#define CATAPULT_FN_POW_NEG_INV 5
-catapult_status catapult_math_probe(int32_t fn, int64_t n, const double *d_a, const double *d_b,
-                                    double *d_out0, double *d_out1, void *stream);
 
 const char *catapult_last_error(void);
 const char *catapult_version(void);

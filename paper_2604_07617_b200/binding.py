@@ -14,28 +14,33 @@ import numpy as np
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libcatapult.so")
+PROBE_LIB_PATH = os.path.join(_PKG, "libcatapult_probe.so")
 
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, 1, 2, 3, 4
 COORD_BOOZER, COORD_CYL = 0, 1
 ST_REACHED_T, ST_LOST, ST_STALLED, ST_MAXSTEPS = 0, 1, 2, 3
-COUNTER_NAMES = ["accepted", "rejected", "reached_T", "lost", "stalled", "max_steps", "rhs_evals", "cell_loads"]
+NCOUNTERS = 10
+COUNTER_NAMES = ["accepted", "rejected", "reached_T", "lost", "stalled", "max_steps", "rhs_evals", "cell_fetches",
+                 "blocking_fetches", "rounds"]
 
 EXPORTS = [
     "catapult_field_build", "catapult_field_build_host", "catapult_field_destroy",
     "catapult_field_table_bytes", "catapult_field_eval", "catapult_field_export_rows",
     "catapult_trace", "catapult_trace_init", "catapult_trace_continue", "catapult_trace_host",
-    "catapult_trace_continue_host", "catapult_trace_scripted",
-    "catapult_step_once", "catapult_estimate", "catapult_math_probe", "catapult_measure_fp64_peak",
-    "catapult_measure_l2_bandwidth", "catapult_trace_launch_shape", "catapult_last_error",
+    "catapult_trace_continue_host", "catapult_release_host_cache", "catapult_trace_scripted",
+    "catapult_step_once", "catapult_estimate", "catapult_trace_launch_shape", "catapult_last_error",
     "catapult_version",
 ]
+PROBE_EXPORTS = ["catapult_math_probe", "catapult_measure_fp64_peak", "catapult_measure_l2_bandwidth",
+                 "catapult_probe_last_error"]
 
 
 class FieldDesc(C.Structure):
     _fields_ = [("coord", C.c_int32), ("ncell", C.c_int32 * 3), ("nfp", C.c_int32),
-                ("nquant", C.c_int32), ("lo", C.c_double * 3), ("hi", C.c_double * 3),
+                ("nquant", C.c_int32), ("quant", C.c_int32 * 16), ("lo", C.c_double * 3), ("hi", C.c_double * 3),
                 ("G0", C.c_double), ("I0", C.c_double), ("iota0", C.c_double),
-                ("iota1", C.c_double), ("psi0", C.c_double)]
+                ("iota1", C.c_double), ("psi0", C.c_double), ("G_nodes", C.c_void_p), ("I_nodes", C.c_void_p),
+                ("iota_nodes", C.c_void_p)]
 
 
 class TraceParams(C.Structure):
@@ -54,6 +59,7 @@ class CatapultError(RuntimeError):
 
 
 _lib = None
+_probe = None
 
 
 def load():
@@ -81,9 +87,7 @@ def load():
     L.catapult_trace_scripted.argtypes = [vp, C.POINTER(TraceParams), i64, dp, C.c_int32, dp, dp, dp, dp, dp, vp]
     L.catapult_step_once.argtypes = [vp, C.POINTER(TraceParams), i64, dp, dp, dp, dp, dp, dp, vp]
     L.catapult_estimate.argtypes = [C.c_int32, i64, dp, dp, dp, dp, dp, vp]
-    L.catapult_math_probe.argtypes = [C.c_int32, i64, dp, dp, dp, dp, vp]
-    L.catapult_measure_fp64_peak.argtypes = [C.POINTER(C.c_double)]
-    L.catapult_measure_l2_bandwidth.argtypes = [C.c_size_t, C.POINTER(C.c_double)]
+    L.catapult_release_host_cache.argtypes = []
     L.catapult_trace_launch_shape.argtypes = [vp, C.POINTER(TraceParams), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     L.catapult_last_error.restype = C.c_char_p
     L.catapult_version.restype = C.c_char_p
@@ -95,9 +99,31 @@ def load():
     return L
 
 
+def load_probe():
+    """Loads libcatapult_probe.so: measurement / test hooks (include/catapult_probe.h), not the product."""
+    global _probe
+    if _probe is not None:
+        return _probe
+    if not os.path.exists(PROBE_LIB_PATH):
+        raise ImportError(f"{PROBE_LIB_PATH} is missing: run `python -m paper_2604_07617_b200.build`")
+    P = C.CDLL(PROBE_LIB_PATH)
+    dp = C.c_void_p
+    P.catapult_math_probe.argtypes = [C.c_int32, C.c_int64, dp, dp, dp, dp, C.c_void_p]
+    P.catapult_measure_fp64_peak.argtypes = [C.POINTER(C.c_double)]
+    P.catapult_measure_l2_bandwidth.argtypes = [C.c_size_t, C.POINTER(C.c_double)]
+    P.catapult_probe_last_error.restype = C.c_char_p
+    _probe = P
+    return P
+
+
 def _check(st: int):
     if st != OK:
         raise CatapultError(st, load().catapult_last_error().decode())
+
+
+def _check_probe(st: int):
+    if st != OK:
+        raise CatapultError(st, load_probe().catapult_probe_last_error().decode())
 
 
 def make_desc(fd: dict) -> FieldDesc:
@@ -111,6 +137,11 @@ def make_desc(fd: dict) -> FieldDesc:
     d.nquant = int(fd["nquant"])
     for k in ("G0", "I0", "iota0", "iota1", "psi0"):
         setattr(d, k, float(fd.get(k, 0.0)))
+    for i, tag in enumerate(fd.get("quant", ())):
+        d.quant[i] = int(tag)
+    for k in ("G_nodes", "I_nodes", "iota_nodes"):        # device pointers (CUDA tensors) or absent
+        t = fd.get(k)
+        setattr(d, k, None if t is None else t.data_ptr())
     return d
 
 
@@ -235,7 +266,7 @@ def catapult_trace(f: Field, pd: dict, d_x0, counters: bool = True) -> dict:
     status = torch.empty(n, dtype=torch.int32, device=dev)
     nacc = torch.empty(n, dtype=torch.int32, device=dev)
     nrej = torch.empty(n, dtype=torch.int32, device=dev)
-    cnt = torch.zeros(8, dtype=torch.int64, device=dev) if counters else None
+    cnt = torch.zeros(NCOUNTERS, dtype=torch.int64, device=dev) if counters else None
     _check(load().catapult_trace(f._h, C.byref(p), n, _ptr(d_x0, torch.float64), _ptr(xf), _ptr(tstop),
                                  _ptr(status), _ptr(nacc), _ptr(nrej), _ptr(cnt, allow_none=True), _stream()))
     return dict(xf=xf, tstop=tstop, status=status, nacc=nacc, nrej=nrej, counters=cnt)
@@ -252,7 +283,7 @@ def catapult_trace_init(f: Field, pd: dict, d_x) -> dict:
               status=torch.empty(n, dtype=torch.int32, device=dev),
               nacc=torch.zeros(n, dtype=torch.int32, device=dev),
               nrej=torch.zeros(n, dtype=torch.int32, device=dev),
-              counters=torch.zeros(8, dtype=torch.int64, device=dev))
+              counters=torch.zeros(NCOUNTERS, dtype=torch.int64, device=dev))
     _check(load().catapult_trace_init(f._h, C.byref(p), n, _ptr(d_x, torch.float64), _ptr(st["t"]), _ptr(st["dt"]),
                                       _ptr(st["mu"]), _ptr(st["status"]), _stream()))
     return st
@@ -276,7 +307,7 @@ def catapult_trace_host(f: Field, pd: dict, h_x0: np.ndarray, out: dict | None =
     if out is None:
         out = dict(xf=np.empty((4, n)), tstop=np.empty(n), status=np.empty(n, dtype=np.int32),
                    nacc=np.empty(n, dtype=np.uint32), nrej=np.empty(n, dtype=np.uint32),
-                   counters=np.zeros(8, dtype=np.uint64))
+                   counters=np.zeros(NCOUNTERS, dtype=np.uint64))
     _check(load().catapult_trace_host(f._h, C.byref(p), n, _hptr(h_x0, np.float64), _hptr(out["xf"], np.float64),
                                       _hptr(out["tstop"], np.float64), _hptr(out["status"], np.int32),
                                       _hptr(out["nacc"], np.uint32), _hptr(out["nrej"], np.uint32),
@@ -286,7 +317,7 @@ def catapult_trace_host(f: Field, pd: dict, h_x0: np.ndarray, out: dict | None =
 
 def catapult_trace_continue_host(f: Field, pd: dict, st: dict) -> dict:
     """HOST-buffer continue: st holds numpy arrays x[4][n], t, dt, mu (float64), status (int32),
-    nacc, nrej (uint32), counters (uint64[8]); all updated in place."""
+    nacc, nrej (uint32), counters (uint64[NCOUNTERS]); all updated in place."""
     p = make_params(pd)
     n = st["x"].shape[1]
     _check(load().catapult_trace_continue_host(
@@ -345,21 +376,25 @@ def catapult_math_probe(fn: int, d_a, d_b=None):
     """Test hook: (out0, out1) of the device-side elementary function `fn` on CUDA float64 tensors."""
     torch = _torch()
     o0, o1 = torch.empty_like(d_a), torch.empty_like(d_a)
-    _check(load().catapult_math_probe(fn, d_a.numel(), _ptr(d_a, torch.float64), _ptr(d_b, torch.float64, True),
-                                      _ptr(o0), _ptr(o1), _stream()))
+    _check_probe(load_probe().catapult_math_probe(fn, d_a.numel(), _ptr(d_a, torch.float64),
+                                                  _ptr(d_b, torch.float64, True), _ptr(o0), _ptr(o1), _stream()))
     return o0, o1
 
 
 def catapult_measure_fp64_peak() -> float:
     v = C.c_double(0)
-    _check(load().catapult_measure_fp64_peak(C.byref(v)))
+    _check_probe(load_probe().catapult_measure_fp64_peak(C.byref(v)))
     return v.value
 
 
 def catapult_measure_l2_bandwidth(nbytes: int) -> float:
     v = C.c_double(0)
-    _check(load().catapult_measure_l2_bandwidth(nbytes, C.byref(v)))
+    _check_probe(load_probe().catapult_measure_l2_bandwidth(nbytes, C.byref(v)))
     return v.value
+
+
+def catapult_release_host_cache():
+    _check(load().catapult_release_host_cache())
 
 
 def catapult_trace_launch_shape(f: Field, pd: dict):

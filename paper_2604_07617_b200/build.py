@@ -1,5 +1,9 @@
-"""Builds paper_2604_07617_b200/libcatapult.so (the C-ABI library of include/catapult.h) in-tree
-with nvcc for sm_100a.  nvcc cross-compiles without a GPU."""
+"""Builds the two shared libraries in-tree with nvcc for sm_100a (nvcc cross-compiles without a GPU):
+
+  paper_2604_07617_b200/libcatapult.so        the product: the C-ABI of include/catapult.h
+  paper_2604_07617_b200/libcatapult_probe.so  measurement / test hooks of include/catapult_probe.h
+                                              (DFMA and L2 peak micro-benchmarks, device math probe)
+"""
 from __future__ import annotations
 
 import os
@@ -12,15 +16,17 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 INC = os.path.join(ROOT, "include")
 LIB = os.path.join(PKG, "libcatapult.so")
+PROBE_LIB = os.path.join(PKG, "libcatapult_probe.so")
 OBJ = os.path.join(PKG, "build")
-SOURCES = ["api.cu", "field.cu", "tracer.cu", "estimate.cu", "peaks.cu", "mathprobe.cu"]
+SOURCES = ["api.cu", "field.cu", "tracer.cu", "estimate.cu"]
+PROBE_SOURCES = ["probe_api.cu", "peaks.cu", "mathprobe.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-         "-Xcompiler", "-fPIC", "-I", INC, "-I", CSRC]
+ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
+FLAGS = ["-O3", "-std=c++17", *ARCH, "-lineinfo", "-Xcompiler", "-fPIC", "-I", INC, "-I", CSRC]
 
 
 def _deps():
-    out = [os.path.join(INC, "catapult.h")]
+    out = [os.path.join(INC, fn) for fn in os.listdir(INC)]
     for fn in os.listdir(CSRC):
         out.append(os.path.join(CSRC, fn))
     return out
@@ -28,11 +34,10 @@ def _deps():
 
 def build(force: bool = False, verbose: bool = False) -> str:
     newest = max(os.path.getmtime(p) for p in _deps())
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
+    if (not force and all(os.path.exists(l) and os.path.getmtime(l) >= newest for l in (LIB, PROBE_LIB))):
         return LIB
     os.makedirs(OBJ, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
-    extra += os.environ.get("CATAPULT_NVCC_FLAGS", "").split()     # e.g. -DCATAPULT_SPLIT_NREG_BOOZER=24 for sweeps
 
     def compile_one(src):
         obj = os.path.join(OBJ, src.replace(".cu", ".o"))
@@ -46,10 +51,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
             raise RuntimeError(f"nvcc failed for {src}")
         return obj
 
-    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
-        objs = list(ex.map(compile_one, SOURCES))
-    cmd = [NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB, *objs]
-    subprocess.run(cmd, check=True)
+    with ThreadPoolExecutor(max_workers=len(SOURCES) + len(PROBE_SOURCES)) as ex:
+        objs = list(ex.map(compile_one, SOURCES + PROBE_SOURCES))
+    n = len(SOURCES)
+    subprocess.run([NVCC, "-shared", *ARCH, "-o", LIB, *objs[:n]], check=True)
+    subprocess.run([NVCC, "-shared", *ARCH, "-o", PROBE_LIB, *objs[n:]], check=True)
     return LIB
 
 

@@ -1,5 +1,6 @@
 // C-ABI entry points of libcatapult.so (include/catapult.h): argument validation, table ownership,
 // parameter packing and stream-ordered launches.  No arithmetic of the method lives here.
+#include <climits>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -25,22 +26,40 @@ static catapult_status fail(catapult_status st, const char* msg) {
   return st;
 }
 
-static const double E_CHARGE = 1.602176634e-19;
 static const double PI = 3.14159265358979323846;
 
 static catapult_status validate_desc(const catapult_field_desc* d) {
   if (!d) return fail(CATAPULT_EINVAL, "desc is NULL");
   if (d->coord != CATAPULT_COORD_BOOZER && d->coord != CATAPULT_COORD_CYL)
     return fail(CATAPULT_EINVAL, "desc.coord must be CATAPULT_COORD_BOOZER or CATAPULT_COORD_CYL");
+  long long ncells = 1;
   for (int i = 0; i < 3; ++i) {
     if (d->ncell[i] < 1) return fail(CATAPULT_EINVAL, "desc.ncell must be >= 1");
     if (!(std::isfinite(d->lo[i]) && std::isfinite(d->hi[i]) && d->hi[i] > d->lo[i]))
       return fail(CATAPULT_EINVAL, "desc.lo/hi must be finite with hi > lo");
+    // the kernels carry a flat cell index in 32 bits and node indices 3*ncell+1 per dimension
+    if (d->ncell[i] > (INT32_MAX - 1) / 3) return fail(CATAPULT_EINVAL, "desc.ncell is too large");
+    ncells *= d->ncell[i];
+    if (ncells > (long long)INT32_MAX) return fail(CATAPULT_EINVAL, "desc.ncell: more than 2^31-1 cells");
   }
   const int want = d->coord == CATAPULT_COORD_BOOZER ? CATAPULT_NQUANT_BOOZER : CATAPULT_NQUANT_CYL;
   if (d->nquant != want) return fail(CATAPULT_EINVAL, "desc.nquant does not match desc.coord (4 Boozer, 7 cyl)");
+  // semantic tags of the columns: all zero = the canonical order of `coord`; anything else must spell it out
+  bool tagged = false;
+  for (int i = 0; i < 16; ++i) tagged = tagged || d->quant[i] != 0;
+  if (tagged) {
+    static const int32_t BZ[4] = {CATAPULT_Q_MODB, CATAPULT_Q_DMODB_DS, CATAPULT_Q_DMODB_DTHETA, CATAPULT_Q_DMODB_DZETA};
+    static const int32_t CY[7] = {CATAPULT_Q_B_R,        CATAPULT_Q_B_PHI,    CATAPULT_Q_B_Z,      CATAPULT_Q_DMODB_DR,
+                                  CATAPULT_Q_DMODB_DPHI_OVER_R, CATAPULT_Q_DMODB_DZ, CATAPULT_Q_PSI_LEVEL};
+    const int32_t* canon = d->coord == CATAPULT_COORD_BOOZER ? BZ : CY;
+    for (int i = 0; i < 16; ++i)
+      if (d->quant[i] != (i < want ? canon[i] : 0))
+        return fail(CATAPULT_EUNSUPPORTED, "desc.quant: only the canonical column order of `coord` is built");
+  }
   if (d->nfp < 1) return fail(CATAPULT_EINVAL, "desc.nfp must be >= 1");
   if (d->coord == CATAPULT_COORD_BOOZER) {
+    if (d->G_nodes || d->I_nodes || d->iota_nodes)
+      return fail(CATAPULT_EUNSUPPORTED, "tabulated G(s) / I(s) / iota(s) profiles are not built (use the scalars)");
     if (d->I0 != 0.0) return fail(CATAPULT_EUNSUPPORTED, "non-vacuum Boozer (I0 != 0) is not built");
     if (!(std::isfinite(d->G0) && d->G0 != 0.0)) return fail(CATAPULT_EINVAL, "desc.G0 must be finite, non-zero");
     if (!(std::isfinite(d->psi0) && d->psi0 != 0.0)) return fail(CATAPULT_EINVAL, "desc.psi0 must be finite, non-zero");
@@ -50,8 +69,10 @@ static catapult_status validate_desc(const catapult_field_desc* d) {
   return CATAPULT_OK;
 }
 
-static void fill_field_const(const catapult_field_desc& d, const double* table, FieldConst* fc) {
+static void fill_field_const(const catapult_field_desc& d, const double* table, const double* node0,
+                             FieldConst* fc) {
   fc->table = table;
+  fc->node0 = node0;
   fc->coord = d.coord;
   fc->m = d.nquant;
   for (int i = 0; i < 3; ++i) {
@@ -100,25 +121,18 @@ static catapult_status make_trace_const(const catapult_field* f, const catapult_
   tc->T = p->T;
   tc->rtol = p->rtol;
   tc->atol = p->atol;
-  // DESIGN.md S3 defaults: dtmax = (pi/2) L / v_total, dt0 = 1e-3 dtmax
-  double dtmax = p->dtmax;
+  // DESIGN.md S3 defaults: dtmax = (pi/2) L / v_total, dt0 = 1e-3 dtmax.  Boozer: L = |G| / |B|(node 0); the
+  // node value is on the device (field_build_kernel leaves it next to the table), so dtmax <= 0 is passed on
+  // and the tracer kernel resolves both defaults itself -- no host read-back, no synchronisation.
+  double dtmax = p->dtmax, dt0 = p->dt0;
   if (!(dtmax > 0.0)) {
-    double L;
-    if (f->desc.coord == CATAPULT_COORD_BOOZER) {
-      // |B| at the first node = the first cell's polynomial at w = (-1,-1,-1) (gc_device.cuh basis)
-      double c[64];
-      cudaError_t e = cudaMemcpy(c, f->d_table, sizeof(c), cudaMemcpyDeviceToHost);
-      if (e != cudaSuccess) return cuda_fail(e, "reading |B|(node 0) for the default dtmax");
-      double b00 = 0.0;
-      for (int i = 0; i < 64; ++i) b00 += (((i >> 4) + ((i >> 2) & 3) + (i & 3)) & 1) ? -c[coef_pos(i)] : c[coef_pos(i)];
-      L = std::fabs(f->desc.G0) / std::fabs(b00);
-    } else {
-      L = f->desc.hi[0];
-    }
-    dtmax = 0.5 * PI * L / tc->vtot;
+    if (f->desc.coord == CATAPULT_COORD_CYL) dtmax = 0.5 * PI * f->desc.hi[0] / tc->vtot;  // L = R_max
+    else dtmax = 0.0;
   }
-  double dt0 = p->dt0 > 0.0 ? p->dt0 : 1e-3 * dtmax;
-  if (dt0 > dtmax) dt0 = dtmax;
+  if (dtmax > 0.0) {
+    dt0 = dt0 > 0.0 ? dt0 : 1e-3 * dtmax;
+    if (dt0 > dtmax) dt0 = dtmax;
+  }
   tc->dt0 = dt0;
   tc->dtmax = dtmax;
   tc->max_steps = p->max_steps;
@@ -131,10 +145,17 @@ static catapult_status make_trace_const(const catapult_field* f, const catapult_
   tc->saw_omega = p->saw_omega;
   tc->saw_inv_omG = p->saw_on ? f->fc.invG / p->saw_omega : 0.0;
   *model = f->desc.coord == CATAPULT_COORD_CYL ? MODEL_CART : (p->saw_on ? MODEL_BOOZER_SAW : MODEL_BOOZER_VAC);
-  (void)E_CHARGE;
   return CATAPULT_OK;
 }
 
+// Every call that reads the tables on `s` is ordered after the build, whatever stream the build ran on.
+static catapult_status use_field_on(const catapult_field* f, cudaStream_t s) {
+  int dev = -1;
+  CATAPULT_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev != f->device) return fail(CATAPULT_EINVAL, "field was built on another device than the current one");
+  CATAPULT_CUDA_TRY(cudaStreamWaitEvent(s, f->built, 0));
+  return CATAPULT_OK;
+}
 static catapult_status use_device_of(const catapult_field* f) {
   int dev = -1;
   CATAPULT_CUDA_TRY(cudaGetDevice(&dev));
@@ -164,15 +185,24 @@ catapult_status catapult_field_build(const catapult_field_desc* desc, const doub
   f->ncells = (int64_t)desc->ncell[0] * desc->ncell[1] * desc->ncell[2];
   f->table_bytes = (size_t)f->ncells * desc->nquant * 64 * sizeof(double);
   f->d_table = nullptr;
+  f->built = nullptr;
+  // stream-ordered allocation: the build neither blocks the host nor synchronises the device
   cudaError_t e = cudaGetDevice(&f->device);
-  if (e == cudaSuccess) e = cudaMalloc((void**)&f->d_table, f->table_bytes);
+  if (e == cudaSuccess) e = cudaMallocAsync((void**)&f->d_table, f->table_bytes + sizeof(double), (cudaStream_t)stream);
   if (e != cudaSuccess) {
     delete f;
-    return cuda_fail(e, "cudaMalloc(table)");
+    return cuda_fail(e, "cudaMallocAsync(table)");
   }
-  fill_field_const(*desc, f->d_table, &f->fc);
-  st = launch_field_build(*desc, d_nodes, f->d_table, (cudaStream_t)stream);
+  double* d_node0 = f->d_table + f->table_bytes / sizeof(double);
+  fill_field_const(*desc, f->d_table, d_node0, &f->fc);
+  st = launch_field_build(*desc, d_nodes, f->d_table, d_node0, (cudaStream_t)stream);
+  if (st == CATAPULT_OK) {
+    e = cudaEventCreateWithFlags(&f->built, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventRecord(f->built, (cudaStream_t)stream);
+    if (e != cudaSuccess) st = cuda_fail(e, "cudaEventRecord(built)");
+  }
   if (st != CATAPULT_OK) {
+    if (f->built) cudaEventDestroy(f->built);
     cudaFree(f->d_table);
     delete f;
     return st;
@@ -209,6 +239,7 @@ catapult_status catapult_field_build_host(const catapult_field_desc* desc, const
 
 catapult_status catapult_field_destroy(catapult_field* f) {
   if (!f) return CATAPULT_OK;
+  if (f->built) cudaEventDestroy(f->built);
   if (f->d_table) cudaFree(f->d_table);
   delete f;
   return CATAPULT_OK;
@@ -221,14 +252,14 @@ catapult_status catapult_field_eval(const catapult_field* f, int64_t npts, const
   if (!f) return fail(CATAPULT_EINVAL, "field is NULL");
   if (npts < 0) return fail(CATAPULT_EINVAL, "npts < 0");
   if (npts > 0 && (!d_pts || !d_out)) return fail(CATAPULT_EINVAL, "d_pts/d_out is NULL");
-  catapult_status st = use_device_of(f);
+  catapult_status st = use_field_on(f, (cudaStream_t)stream);
   if (st != CATAPULT_OK) return st;
   return launch_field_eval(f->fc, npts, d_pts, d_out, (cudaStream_t)stream);
 }
 
 catapult_status catapult_field_export_rows(const catapult_field* f, double* d_out, void* stream) {
   if (!f || !d_out) return fail(CATAPULT_EINVAL, "field/d_out is NULL");
-  catapult_status st = use_device_of(f);
+  catapult_status st = use_field_on(f, (cudaStream_t)stream);
   if (st != CATAPULT_OK) return st;
   return launch_field_export_rows(f->fc, f->ncells, d_out, (cudaStream_t)stream);
 }
@@ -239,7 +270,7 @@ static catapult_status run_trace(const catapult_field* f, const catapult_trace_p
   int model = 0;
   catapult_status st = make_trace_const(f, p, &tc, &model);
   if (st != CATAPULT_OK) return st;
-  st = use_device_of(f);
+  st = use_field_on(f, s);
   if (st != CATAPULT_OK) return st;
   if (a.n == 0) return CATAPULT_OK;
   unsigned long long* queue = nullptr;
@@ -330,6 +361,54 @@ catapult_status catapult_trace_continue(const catapult_field* f, const catapult_
   return run_trace(f, p, a, (cudaStream_t)stream);
 }
 
+// ---- HOST-buffer forms -------------------------------------------------------------------------------------
+// One staging slab and one non-blocking stream per host thread, kept between calls (grown on demand, released
+// by catapult_release_host_cache): the copies and the kernel are enqueued back to back on that stream and the
+// call returns after one cudaStreamSynchronize.
+namespace {
+struct HostCache {
+  int device = -1;
+  cudaStream_t stream = nullptr;
+  char* slab = nullptr;
+  size_t bytes = 0;
+  void release() {
+    if (slab) cudaFree(slab);
+    if (stream) cudaStreamDestroy(stream);
+    slab = nullptr;
+    stream = nullptr;
+    bytes = 0;
+    device = -1;
+  }
+  ~HostCache() {}  // at thread exit the CUDA context may be gone already: nothing is freed here
+};
+thread_local HostCache g_host;
+
+catapult_status host_slab(const catapult_field* f, size_t bytes, char** slab, cudaStream_t* stream) {
+  catapult_status st = use_device_of(f);
+  if (st != CATAPULT_OK) return st;
+  if (g_host.device != f->device) g_host.release();
+  if (!g_host.stream) {
+    CATAPULT_CUDA_TRY(cudaStreamCreateWithFlags(&g_host.stream, cudaStreamNonBlocking));
+    g_host.device = f->device;
+  }
+  if (g_host.bytes < bytes) {
+    if (g_host.slab) cudaFree(g_host.slab);
+    g_host.slab = nullptr;
+    g_host.bytes = 0;
+    CATAPULT_CUDA_TRY(cudaMalloc((void**)&g_host.slab, bytes));
+    g_host.bytes = bytes;
+  }
+  *slab = g_host.slab;
+  *stream = g_host.stream;
+  return CATAPULT_OK;
+}
+}  // namespace
+
+catapult_status catapult_release_host_cache(void) {
+  g_host.release();
+  return CATAPULT_OK;
+}
+
 catapult_status catapult_trace_host(const catapult_field* f, const catapult_trace_params* p, int64_t n,
                                     const double* h_x0, double* h_xf, double* h_tstop, int32_t* h_status,
                                     uint32_t* h_nacc, uint32_t* h_nrej, uint64_t* h_counters) {
@@ -338,37 +417,36 @@ catapult_status catapult_trace_host(const catapult_field* f, const catapult_trac
     return fail(CATAPULT_EINVAL, "h_x0, h_xf, h_tstop and h_status are required");
   if (!f || !p) return fail(CATAPULT_EINVAL, "field/params is NULL");
   if (n == 0) return CATAPULT_OK;
-  // one device slab: x0[4n] xf[4n] tstop[n] | status[n] nacc[n] nrej[n] | counters[8]
+  // one device slab: x0[4n] xf[4n] tstop[n] | counters | status[n] nacc[n] nrej[n]
   const size_t nd = (size_t)n;
-  const size_t bytes = nd * 9 * sizeof(double) + nd * 3 * sizeof(uint32_t) + 8 * sizeof(uint64_t) + 64;
+  const size_t bytes = nd * 9 * sizeof(double) + CATAPULT_NCOUNTERS * sizeof(uint64_t) + nd * 3 * sizeof(uint32_t) + 64;
   char* slab = nullptr;
-  CATAPULT_CUDA_TRY(cudaMalloc((void**)&slab, bytes));
+  cudaStream_t s = nullptr;
+  catapult_status st = host_slab(f, bytes, &slab, &s);
+  if (st != CATAPULT_OK) return st;
   double* d_x0 = (double*)slab;
   double* d_xf = d_x0 + 4 * nd;
   double* d_ts = d_xf + 4 * nd;
   uint64_t* d_cnt = (uint64_t*)(d_ts + nd);
-  int32_t* d_st = (int32_t*)(d_cnt + 8);
+  int32_t* d_st = (int32_t*)(d_cnt + CATAPULT_NCOUNTERS);
   uint32_t* d_na = (uint32_t*)(d_st + nd);
   uint32_t* d_nr = d_na + nd;
-  catapult_status st = CATAPULT_OK;
-  cudaError_t e = cudaMemcpyAsync(d_x0, h_x0, 4 * nd * sizeof(double), cudaMemcpyHostToDevice, 0);
-  if (e == cudaSuccess) e = cudaMemsetAsync(d_cnt, 0, 8 * sizeof(uint64_t), 0);
+  const cudaMemcpyKind H2D = cudaMemcpyHostToDevice, D2H = cudaMemcpyDeviceToHost;
+  cudaError_t e = cudaMemcpyAsync(d_x0, h_x0, 4 * nd * sizeof(double), H2D, s);
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_cnt, 0, CATAPULT_NCOUNTERS * sizeof(uint64_t), s);
   if (e == cudaSuccess) {
-    st = catapult_trace(f, p, n, d_x0, d_xf, d_ts, d_st, d_na, d_nr, d_cnt, nullptr);
+    st = catapult_trace(f, p, n, d_x0, d_xf, d_ts, d_st, d_na, d_nr, d_cnt, s);
     if (st == CATAPULT_OK) {
-      e = cudaMemcpyAsync(h_xf, d_xf, 4 * nd * sizeof(double), cudaMemcpyDeviceToHost, 0);
-      if (e == cudaSuccess) e = cudaMemcpyAsync(h_tstop, d_ts, nd * sizeof(double), cudaMemcpyDeviceToHost, 0);
-      if (e == cudaSuccess) e = cudaMemcpyAsync(h_status, d_st, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, 0);
-      if (e == cudaSuccess && h_nacc)
-        e = cudaMemcpyAsync(h_nacc, d_na, nd * sizeof(uint32_t), cudaMemcpyDeviceToHost, 0);
-      if (e == cudaSuccess && h_nrej)
-        e = cudaMemcpyAsync(h_nrej, d_nr, nd * sizeof(uint32_t), cudaMemcpyDeviceToHost, 0);
+      e = cudaMemcpyAsync(h_xf, d_xf, 4 * nd * sizeof(double), D2H, s);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h_tstop, d_ts, nd * sizeof(double), D2H, s);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h_status, d_st, nd * sizeof(int32_t), D2H, s);
+      if (e == cudaSuccess && h_nacc) e = cudaMemcpyAsync(h_nacc, d_na, nd * sizeof(uint32_t), D2H, s);
+      if (e == cudaSuccess && h_nrej) e = cudaMemcpyAsync(h_nrej, d_nr, nd * sizeof(uint32_t), D2H, s);
       if (e == cudaSuccess && h_counters)
-        e = cudaMemcpyAsync(h_counters, d_cnt, 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost, 0);
+        e = cudaMemcpyAsync(h_counters, d_cnt, CATAPULT_NCOUNTERS * sizeof(uint64_t), D2H, s);
     }
   }
-  cudaError_t e2 = cudaStreamSynchronize(0);
-  cudaFree(slab);
+  cudaError_t e2 = cudaStreamSynchronize(s);
   if (st != CATAPULT_OK) return st;
   if (e != cudaSuccess) return cuda_fail(e, "catapult_trace_host copies");
   if (e2 != cudaSuccess) return cuda_fail(e2, "catapult_trace_host");
@@ -383,47 +461,47 @@ catapult_status catapult_trace_continue_host(const catapult_field* f, const cata
     return fail(CATAPULT_EINVAL, "h_x, h_t, h_dt, h_mu and h_status are required");
   if (!f || !p) return fail(CATAPULT_EINVAL, "field/params is NULL");
   if (n == 0) return CATAPULT_OK;
-  // one device slab: x[4n] t[n] dt[n] mu[n] | counters[8] | status[n] nacc[n] nrej[n]
+  // one device slab: x[4n] t[n] dt[n] mu[n] | counters | status[n] nacc[n] nrej[n]
   const size_t nd = (size_t)n;
-  const size_t bytes = nd * 7 * sizeof(double) + 8 * sizeof(uint64_t) + nd * 3 * sizeof(uint32_t) + 64;
+  const size_t bytes = nd * 7 * sizeof(double) + CATAPULT_NCOUNTERS * sizeof(uint64_t) + nd * 3 * sizeof(uint32_t) + 64;
   char* slab = nullptr;
-  CATAPULT_CUDA_TRY(cudaMalloc((void**)&slab, bytes));
+  cudaStream_t s = nullptr;
+  catapult_status st = host_slab(f, bytes, &slab, &s);
+  if (st != CATAPULT_OK) return st;
   double* d_x = (double*)slab;
   double* d_t = d_x + 4 * nd;
   double* d_dt = d_t + nd;
   double* d_mu = d_dt + nd;
   uint64_t* d_cnt = (uint64_t*)(d_mu + nd);
-  int32_t* d_st = (int32_t*)(d_cnt + 8);
+  int32_t* d_st = (int32_t*)(d_cnt + CATAPULT_NCOUNTERS);
   uint32_t* d_na = (uint32_t*)(d_st + nd);
   uint32_t* d_nr = d_na + nd;
-  catapult_status st = CATAPULT_OK;
   const cudaMemcpyKind H2D = cudaMemcpyHostToDevice, D2H = cudaMemcpyDeviceToHost;
-  cudaError_t e = cudaMemcpyAsync(d_x, h_x, 4 * nd * sizeof(double), H2D, 0);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(d_t, h_t, nd * sizeof(double), H2D, 0);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(d_dt, h_dt, nd * sizeof(double), H2D, 0);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(d_mu, h_mu, nd * sizeof(double), H2D, 0);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(d_st, h_status, nd * sizeof(int32_t), H2D, 0);
-  if (e == cudaSuccess) e = h_nacc ? cudaMemcpyAsync(d_na, h_nacc, nd * sizeof(uint32_t), H2D, 0)
-                                   : cudaMemsetAsync(d_na, 0, nd * sizeof(uint32_t), 0);
-  if (e == cudaSuccess) e = h_nrej ? cudaMemcpyAsync(d_nr, h_nrej, nd * sizeof(uint32_t), H2D, 0)
-                                   : cudaMemsetAsync(d_nr, 0, nd * sizeof(uint32_t), 0);
-  if (e == cudaSuccess) e = h_counters ? cudaMemcpyAsync(d_cnt, h_counters, 8 * sizeof(uint64_t), H2D, 0)
-                                       : cudaMemsetAsync(d_cnt, 0, 8 * sizeof(uint64_t), 0);
+  const size_t cb = CATAPULT_NCOUNTERS * sizeof(uint64_t);
+  cudaError_t e = cudaMemcpyAsync(d_x, h_x, 4 * nd * sizeof(double), H2D, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_t, h_t, nd * sizeof(double), H2D, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_dt, h_dt, nd * sizeof(double), H2D, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_mu, h_mu, nd * sizeof(double), H2D, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_st, h_status, nd * sizeof(int32_t), H2D, s);
+  if (e == cudaSuccess) e = h_nacc ? cudaMemcpyAsync(d_na, h_nacc, nd * sizeof(uint32_t), H2D, s)
+                                   : cudaMemsetAsync(d_na, 0, nd * sizeof(uint32_t), s);
+  if (e == cudaSuccess) e = h_nrej ? cudaMemcpyAsync(d_nr, h_nrej, nd * sizeof(uint32_t), H2D, s)
+                                   : cudaMemsetAsync(d_nr, 0, nd * sizeof(uint32_t), s);
+  if (e == cudaSuccess) e = h_counters ? cudaMemcpyAsync(d_cnt, h_counters, cb, H2D, s) : cudaMemsetAsync(d_cnt, 0, cb, s);
   if (e == cudaSuccess) {
-    st = catapult_trace_continue(f, p, n, d_x, d_t, d_dt, d_mu, d_st, d_na, d_nr, d_cnt, nullptr);
+    st = catapult_trace_continue(f, p, n, d_x, d_t, d_dt, d_mu, d_st, d_na, d_nr, d_cnt, s);
     if (st == CATAPULT_OK) {
-      e = cudaMemcpyAsync(h_x, d_x, 4 * nd * sizeof(double), D2H, 0);
-      if (e == cudaSuccess) e = cudaMemcpyAsync(h_t, d_t, nd * sizeof(double), D2H, 0);
-      if (e == cudaSuccess) e = cudaMemcpyAsync(h_dt, d_dt, nd * sizeof(double), D2H, 0);
-      if (e == cudaSuccess) e = cudaMemcpyAsync(h_mu, d_mu, nd * sizeof(double), D2H, 0);
-      if (e == cudaSuccess) e = cudaMemcpyAsync(h_status, d_st, nd * sizeof(int32_t), D2H, 0);
-      if (e == cudaSuccess && h_nacc) e = cudaMemcpyAsync(h_nacc, d_na, nd * sizeof(uint32_t), D2H, 0);
-      if (e == cudaSuccess && h_nrej) e = cudaMemcpyAsync(h_nrej, d_nr, nd * sizeof(uint32_t), D2H, 0);
-      if (e == cudaSuccess && h_counters) e = cudaMemcpyAsync(h_counters, d_cnt, 8 * sizeof(uint64_t), D2H, 0);
+      e = cudaMemcpyAsync(h_x, d_x, 4 * nd * sizeof(double), D2H, s);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h_t, d_t, nd * sizeof(double), D2H, s);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h_dt, d_dt, nd * sizeof(double), D2H, s);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h_mu, d_mu, nd * sizeof(double), D2H, s);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h_status, d_st, nd * sizeof(int32_t), D2H, s);
+      if (e == cudaSuccess && h_nacc) e = cudaMemcpyAsync(h_nacc, d_na, nd * sizeof(uint32_t), D2H, s);
+      if (e == cudaSuccess && h_nrej) e = cudaMemcpyAsync(h_nrej, d_nr, nd * sizeof(uint32_t), D2H, s);
+      if (e == cudaSuccess && h_counters) e = cudaMemcpyAsync(h_counters, d_cnt, cb, D2H, s);
     }
   }
-  cudaError_t e2 = cudaStreamSynchronize(0);
-  cudaFree(slab);
+  cudaError_t e2 = cudaStreamSynchronize(s);
   if (st != CATAPULT_OK) return st;
   if (e != cudaSuccess) return cuda_fail(e, "catapult_trace_continue_host copies");
   if (e2 != cudaSuccess) return cuda_fail(e2, "catapult_trace_continue_host");
@@ -440,7 +518,7 @@ catapult_status catapult_step_once(const catapult_field* f, const catapult_trace
   int model = 0;
   catapult_status st = make_trace_const(f, p, &tc, &model);
   if (st != CATAPULT_OK) return st;
-  st = use_device_of(f);
+  st = use_field_on(f, (cudaStream_t)stream);
   if (st != CATAPULT_OK) return st;
   if (n == 0) return CATAPULT_OK;
   TraceArgs a{};
@@ -479,25 +557,6 @@ catapult_status catapult_estimate(int32_t g_kind, int64_t n, const int32_t* d_st
     CATAPULT_CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
   }
   return CATAPULT_OK;
-}
-
-catapult_status catapult_math_probe(int32_t fn, int64_t n, const double* d_a, const double* d_b, double* d_out0,
-                                    double* d_out1, void* stream) {
-  if (n < 0) return fail(CATAPULT_EINVAL, "n < 0");
-  if (fn < 0 || fn > CATAPULT_FN_POW_NEG_INV) return fail(CATAPULT_EINVAL, "unknown fn");
-  if (n > 0 && (!d_a || !d_out0)) return fail(CATAPULT_EINVAL, "d_a/d_out0 is NULL");
-  if (n > 0 && fn == CATAPULT_FN_ATAN2 && !d_b) return fail(CATAPULT_EINVAL, "atan2 needs d_b");
-  return launch_math_probe(fn, n, d_a, d_b, d_out0, d_out1, (cudaStream_t)stream);
-}
-
-catapult_status catapult_measure_fp64_peak(double* flops_per_s) {
-  if (!flops_per_s) return fail(CATAPULT_EINVAL, "flops_per_s is NULL");
-  return measure_fp64_peak(flops_per_s);
-}
-
-catapult_status catapult_measure_l2_bandwidth(size_t bytes, double* bytes_per_s) {
-  if (!bytes_per_s) return fail(CATAPULT_EINVAL, "bytes_per_s is NULL");
-  return measure_l2_bandwidth(bytes, bytes_per_s);
 }
 
 catapult_status catapult_trace_launch_shape(const catapult_field* f, const catapult_trace_params* p, int32_t* blocks,

@@ -42,9 +42,12 @@ __device__ __forceinline__ void nodal_to_monomial(dd& f0, dd& f1, dd& f2, dd& f3
 
 // One thread per (cell, quantity): gathers the 4x4x4 nodal block nodes[q][3*i0+a][3*i1+b][3*i2+c] (shared faces
 // are read by both neighbours), changes basis along the three axes, writes 512 contiguous bytes
-// table[(cell*m + q)*64 + coef_pos((i*4+j)*4+k)] (gc_device.cuh: register half first, shared half second).
+// table[(cell*m + q)*64 + coef_pos(boozer, p0, p1, p2)] (gc_device.cuh: coefficient of w0^p0 w1^p1 w2^p2; register
+// half first, shared half second).  The thread of (cell 0, quantity 0) also copies the first node of column 0
+// (|B| on the axis for a Boozer grid) to *node0: DESIGN.md S3's default step length needs it.
 __global__ void __launch_bounds__(128)
-field_build_kernel(const double* __restrict__ nodes, double* __restrict__ table, int m, int k0, int k1, int k2) {
+field_build_kernel(const double* __restrict__ nodes, double* __restrict__ table, double* __restrict__ node0, int m,
+                   int k0, int k1, int k2, int boozer) {
   const long long total = (long long)k0 * k1 * k2 * m;
   const long long n1 = 3LL * k1 + 1, n2 = 3LL * k2 + 1, n0 = 3LL * k0 + 1;
   for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < total;
@@ -74,8 +77,14 @@ field_build_kernel(const double* __restrict__ nodes, double* __restrict__ table,
       }
     }
     double* dst = table + o * 64;
+    if (boozer) {
 #pragma unroll
-    for (int e = 0; e < 64; ++e) dst[coef_pos(e)] = v[e].hi;  // normalised: hi = fl(hi + lo)
+      for (int e = 0; e < 64; ++e) dst[coef_pos(true, e >> 4, (e >> 2) & 3, e & 3)] = v[e].hi;  // hi = fl(hi + lo)
+    } else {
+#pragma unroll
+      for (int e = 0; e < 64; ++e) dst[coef_pos(false, e >> 4, (e >> 2) & 3, e & 3)] = v[e].hi;
+    }
+    if (o == 0) *node0 = nodes[0];
   }
 }
 
@@ -87,21 +96,24 @@ field_eval_kernel(const __grid_constant__ FieldConst f, long long npts, const do
                   double* __restrict__ out) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= npts) return;
+  using AX = AxisRoles<BOOZER>;
   double w[3];
   const int cell = locate<BOOZER>(f, pts[i], pts[npts + i], pts[2 * npts + i], w);
   for (int q = 0; q < f.m; ++q) {
     const double* src = f.table + ((long long)cell * f.m + q) * 64;
     out[(long long)q * npts + i] = horner64(
-        [&](int e, double& f0, double& f1, double& f2, double& f3) { ldg_f64x4(src + coef_pos(e), f0, f1, f2, f3); }, w[0], w[1],
-        w[2]);
+        [&](int e, double& f0, double& f1, double& f2, double& f3) { ldg_f64x4(src + e, f0, f1, f2, f3); },
+        w[AX::LAST], w[AX::SECOND], w[AX::FIRST]);
   }
 }
 
 // test hook: nodal values recovered from the table in the paper's row layout (row = node,
 // column = quantity): out[(cell*64+node)*m + q] = polynomial of (cell,q) at the in-cell node (a,b,c),
 // w = -1, -1/3, 1/3, 1.  Equal to the input nodes up to the rounding of the stored coefficients.
+template <bool BOOZER>
 __global__ void field_export_rows_kernel(const double* __restrict__ table, double* __restrict__ out, int m,
                                          long long ncells) {
+  using AX = AxisRoles<BOOZER>;
   const long long total = ncells * m * 64;
   for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < total;
        o += (long long)gridDim.x * blockDim.x) {
@@ -110,10 +122,11 @@ __global__ void field_export_rows_kernel(const double* __restrict__ table, doubl
     const int node = (int)(row & 63);
     const long long cell = row >> 6;
     const double* src = table + (cell * m + q) * 64;
-    const double wa = ((node >> 4) * 2 - 3) * (1.0 / 3.0), wb = (((node >> 2) & 3) * 2 - 3) * (1.0 / 3.0),
-                 wc = ((node & 3) * 2 - 3) * (1.0 / 3.0);
+    const double w[3] = {((node >> 4) * 2 - 3) * (1.0 / 3.0), (((node >> 2) & 3) * 2 - 3) * (1.0 / 3.0),
+                         ((node & 3) * 2 - 3) * (1.0 / 3.0)};
     out[o] = horner64(
-        [&](int e, double& f0, double& f1, double& f2, double& f3) { ldg_f64x4(src + coef_pos(e), f0, f1, f2, f3); }, wa, wb, wc);
+        [&](int e, double& f0, double& f1, double& f2, double& f3) { ldg_f64x4(src + e, f0, f1, f2, f3); },
+        w[AX::LAST], w[AX::SECOND], w[AX::FIRST]);
   }
 }
 
@@ -124,10 +137,10 @@ static int grid_for(long long total, int threads) {
 }
 
 catapult_status launch_field_build(const catapult_field_desc& d, const double* d_nodes, double* d_table,
-                                   cudaStream_t s) {
+                                   double* d_node0, cudaStream_t s) {
   const long long total = (long long)d.ncell[0] * d.ncell[1] * d.ncell[2] * d.nquant;
-  field_build_kernel<<<grid_for(total, 128), 128, 0, s>>>(d_nodes, d_table, d.nquant, d.ncell[0], d.ncell[1],
-                                                          d.ncell[2]);
+  field_build_kernel<<<grid_for(total, 128), 128, 0, s>>>(d_nodes, d_table, d_node0, d.nquant, d.ncell[0], d.ncell[1],
+                                                          d.ncell[2], d.coord == CATAPULT_COORD_BOOZER);
   CATAPULT_CUDA_TRY(cudaGetLastError());
   return CATAPULT_OK;
 }
@@ -144,7 +157,10 @@ catapult_status launch_field_eval(const FieldConst& fc, int64_t npts, const doub
 
 catapult_status launch_field_export_rows(const FieldConst& fc, int64_t ncells, double* d_out, cudaStream_t s) {
   const long long total = ncells * fc.m * 64;
-  field_export_rows_kernel<<<grid_for(total, 256), 256, 0, s>>>(fc.table, d_out, fc.m, ncells);
+  if (fc.coord == CATAPULT_COORD_BOOZER)
+    field_export_rows_kernel<true><<<grid_for(total, 256), 256, 0, s>>>(fc.table, d_out, fc.m, ncells);
+  else
+    field_export_rows_kernel<false><<<grid_for(total, 256), 256, 0, s>>>(fc.table, d_out, fc.m, ncells);
   CATAPULT_CUDA_TRY(cudaGetLastError());
   return CATAPULT_OK;
 }

@@ -2,11 +2,19 @@
 // the table's basis, the step-size controller, state conversions and the loss test.  fp64 throughout.
 //
 // Table basis: the local tricubic of PAPER.md:47-53 is stored per cell and
-// quantity as its 64 coefficients in the centred monomials w0^i w1^j w2^k, w_d = 2 u_d - 1 in [-1,1]
-// (element (i*4+j)*4+k), not as its 64 nodal values: the interpolant is the same polynomial, its
-// evaluation is a nested Horner scheme of 63 FMA on the three local coordinates alone (no Lagrange
-// basis to build: 84 FMA + ~40 flops).  field.cu converts nodal values to this basis in double-double
-// arithmetic, so every stored coefficient is the exact one rounded once.
+// quantity as its 64 coefficients in the centred monomials of the three local coordinates, w_d = 2 u_d - 1
+// in [-1,1], not as its 64 nodal values: the interpolant is the same polynomial, its evaluation is a
+// nested Horner scheme of 63 FMA on the three local coordinates alone (no Lagrange basis to build:
+// 84 FMA + ~40 flops).  field.cu converts nodal values to this basis in double-double arithmetic, so
+// every stored coefficient is the exact one rounded once.
+//
+// The three grid dimensions play three ROLES in the tracer (tracer.cu), named after the order in which a
+// stage point's coordinates become known to the scalar warp:
+//   FIRST  : the coordinate that is a state variable itself      (Boozer zeta = dim 2; cylindrical Z = dim 1)
+//   SECOND : the one that needs a square root                    (Boozer s = dim 0;    cylindrical R = dim 0)
+//   LAST   : the one that needs an arctangent                    (Boozer theta = dim 1; cylindrical phi = dim 2)
+// Stored element (a*4 + b)*4 + c is the coefficient of wLAST^a wSECOND^b wFIRST^c: a run of four along c is a
+// "row", the contraction runs FIRST -> SECOND -> LAST.
 #pragma once
 
 #include "gc_math.cuh"
@@ -64,47 +72,48 @@ __device__ __forceinline__ int locate(const FieldConst& f, double x0, double x1,
   return flat_cell(f, i[0], i[1], i[2]);
 }
 
-// Storage order of a (cell, quantity) block of 64 coefficients.  Row (i, j) = the 4 coefficients along k of
-// w0^i w1^j.  The rows j = 0, 1 of the four slabs come first (256 bytes: the half a tracer thread keeps in
-// registers), then the rows j = 2, 3 (256 bytes: the half it keeps in shared memory, fetched by ONE bulk copy).
-__host__ __device__ constexpr int coef_row_pos(int row) {  // row = i*4 + j  ->  offset of its 4 coefficients
-  return ((row & 3) < 2 ? 0 : 32) + ((row >> 2) * 2 + (row & 1)) * 4;
+// Which grid dimension plays which role (see the top of this file).
+template <bool BOOZER>
+struct AxisRoles {
+  static constexpr int FIRST = BOOZER ? 2 : 1, SECOND = 0, LAST = BOOZER ? 1 : 2;
+};
+// Storage position of the coefficient of w0^p0 w1^p1 w2^p2 (powers per GRID dimension) inside a (cell, quantity)
+// block of 64.  The first 32 stored coefficients (LAST-power 0, 1: 256 bytes) are the half a tracer thread keeps
+// in registers, the other 32 (LAST-power 2, 3) the half it keeps in shared memory, fetched by ONE bulk copy.
+__host__ __device__ constexpr int coef_pos(bool boozer, int p0, int p1, int p2) {
+  return boozer ? (p1 * 4 + p0) * 4 + p2 : (p2 * 4 + p0) * 4 + p1;
 }
-__host__ __device__ constexpr int coef_pos(int e) { return coef_row_pos(e >> 2) + (e & 3); }  // e = (i*4+j)*4+k
 
 // 256-bit read-only global load (sm_100: LDG.E.256)
 __device__ __forceinline__ void ldg_f64x4(const double* p, double& a, double& b, double& c, double& d) {
   asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
 }
 
-// sum_ijk C[(i*4+j)*4+k] w0^i w1^j w2^k.  get4(e, f0..f3) delivers the coefficients e..e+3 (a run along k) from
-// wherever they live (registers, shared memory, global).  The polynomial is evaluated as U + w1^2 V, where U
-// collects the rows j = 0, 1 and V the rows j = 2, 3 of every slab i (the two halves of the stored block,
-// coef_row_pos): each row by Horner in w2 (3 FMA), the two rows of a slab half by one FMA in w1, the four slabs
-// of a half by Horner in w0, and one last FMA: 48 + 8 + 6 + 1 = 63 FMA and one multiplication.  The two halves
-// are independent of each other, which is what the tracer's contraction warps exploit (tracer.cu); every user
-// of the table evaluates it in this one order.
+// sum_abc C[(a*4+b)*4+c] wL^a wS^b wF^c.  get4(e, f0..f3) delivers the stored coefficients e..e+3 (a row) from
+// wherever they live (registers, shared memory, global).  Every row by Horner in wF (3 FMA), the four rows of
+// one LAST-power a by Horner in wS (3 FMA) -> plane value P_a, the four planes by Horner in wL (3 FMA):
+// 48 + 12 + 3 = 63 FMA.  The tracer's contraction warps compute P_0..P_3 (they need only wF and wS), its
+// scalar warp the last three FMA (tracer.cu); every user of the table evaluates it in this one order.
+__device__ __forceinline__ double horner_row(double f0, double f1, double f2, double f3, double w) {
+  return fma(fma(fma(f3, w, f2), w, f1), w, f0);
+}
 template <class Get4>
-__device__ __forceinline__ double horner64(Get4 get4, double w0, double w1, double w2) {
-  double half[2];
+__device__ __forceinline__ double horner_plane(Get4 get4, int a, double wS, double wF) {
+  double row[4];
 #pragma unroll
-  for (int hh = 0; hh < 2; ++hh) {
-    double acc = 0.0;
-#pragma unroll
-    for (int i = 3; i >= 0; --i) {
-      double row[2];
-#pragma unroll
-      for (int jj = 0; jj < 2; ++jj) {
-        double f0, f1, f2, f3;
-        get4((i * 4 + 2 * hh + jj) * 4, f0, f1, f2, f3);
-        row[jj] = fma(fma(fma(f3, w2, f2), w2, f1), w2, f0);
-      }
-      const double pair = fma(row[1], w1, row[0]);
-      acc = (i == 3) ? pair : fma(acc, w0, pair);
-    }
-    half[hh] = acc;
+  for (int b = 0; b < 4; ++b) {
+    double f0, f1, f2, f3;
+    get4((a * 4 + b) * 4, f0, f1, f2, f3);
+    row[b] = horner_row(f0, f1, f2, f3, wF);
   }
-  return fma(half[1], w1 * w1, half[0]);
+  return horner_row(row[0], row[1], row[2], row[3], wS);
+}
+template <class Get4>
+__device__ __forceinline__ double horner64(Get4 get4, double wL, double wS, double wF) {
+  double P[4];
+#pragma unroll
+  for (int a = 0; a < 4; ++a) P[a] = horner_plane(get4, a, wS, wF);
+  return horner_row(P[0], P[1], P[2], P[3], wL);
 }
 
 // Boost odeint default step adjuster for dopri5 (S2):

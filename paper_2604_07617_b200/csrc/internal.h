@@ -15,6 +15,7 @@ namespace catapult {
 // "Data that is used by all threads is moved to constant memory").
 struct FieldConst {
   const double* table;  // [cell][quantity][64], cell-major (include/catapult.h)
+  const double* node0;  // device scalar: first node of column 0 (written by field_build_kernel)
   int coord, m;
   int k[3];
   double lo[3], invh[3], span[3], invspan[3];
@@ -24,7 +25,7 @@ struct FieldConst {
 struct TraceConst {
   FieldConst f;
   double M, invM, q, Moq, vtot, vtot2;
-  double T, rtol, atol, dt0, dtmax;
+  double T, rtol, atol, dt0, dtmax;  // dt0 / dtmax <= 0: DESIGN.md S3 defaults, resolved on the device
   long long max_steps;
   int max_rej;
   int saw_m, saw_n;
@@ -41,7 +42,7 @@ struct TraceArgs {
   int* status;         // [n]; in only when resume
   unsigned* nacc;      // nullable
   unsigned* nrej;      // nullable
-  unsigned long long* counters;  // nullable, 8 entries
+  unsigned long long* counters;  // nullable, CATAPULT_NCOUNTERS entries
   unsigned long long* queue;     // work counter, zero at launch
   int resume;     // 1: continue from (t,dt,mu,status) arrays
   int init_only;  // 1: only fill (t,dt,mu,status)
@@ -63,7 +64,7 @@ catapult_status cuda_fail(cudaError_t e, const char* what);
 
 // field.cu
 catapult_status launch_field_build(const catapult_field_desc& d, const double* d_nodes, double* d_table,
-                                   cudaStream_t s);
+                                   double* d_node0, cudaStream_t s);
 catapult_status launch_field_eval(const FieldConst& fc, int64_t npts, const double* d_pts, double* d_out,
                                   cudaStream_t s);
 catapult_status launch_field_export_rows(const FieldConst& fc, int64_t ncells, double* d_out, cudaStream_t s);
@@ -89,8 +90,9 @@ catapult_status measure_l2_bandwidth(size_t bytes, double* bps);
 struct catapult_field {
   catapult_field_desc desc;
   catapult::FieldConst fc;
-  double* d_table;
+  double* d_table;   // table_bytes of coefficients, followed by the node0 scalar
   size_t table_bytes;
   int64_t ncells;
   int device;
+  cudaEvent_t built;  // recorded on the build stream after field_build_kernel
 };

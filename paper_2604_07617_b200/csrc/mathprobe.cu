@@ -1,6 +1,7 @@
 // Test hook: evaluates the device-side elementary functions of gc_math.cuh on arrays, so that
 // tests/test_gpu_parity.py can compare them with numpy on the argument ranges the tracer uses.
 #include "gc_math.cuh"
+#include "catapult_probe.h"
 #include "internal.h"
 
 namespace catapult {

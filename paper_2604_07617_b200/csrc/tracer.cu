@@ -1,47 +1,39 @@
-// Persistent fp64 DP5 guiding-centre tracer, warp-specialised ("split") form.
+// Persistent fp64 DP5 guiding-centre tracer: warp-specialised, pipelined along the interpolation axes.
 //
 // What is computed is PAPER.md:57-61 (DESIGN.md sections 1-2); the launch shape is this library's own.
 //
 // A block serves 32 particle slots with NQ + 1 warps (NQ = tabulated quantities: 4 Boozer, 7 cylindrical):
-//   * the SCALAR warp: lane l owns particle slot l -- state, DP5 stage algebra, cell locate, the
-//     guiding-centre physics, error norm, controller, stop test and refill.  Nothing is replicated:
-//     one warp instruction advances 32 particles.
+//   * the SCALAR warp: lane l owns particle slot l -- state, DP5 stage states, cell locate, the guiding-centre
+//     physics, error norm, controller, stop test and refill.  One warp instruction advances 32 particles.
 //   * NQ CONTRACTION warps: lane l of warp q owns the 64 tricubic coefficients of quantity q of slot l's
-//     current cell, on chip (half in registers, half in a private conflict-free run of shared
-//     memory), re-fetched from the cell-major table only when the slot's cell changes.  Per evaluation it
-//     reads the slot's (cell, w) from shared memory, evaluates the 64-coefficient polynomial by nested
-//     Horner (63 FMA, gc_device.cuh) and writes one value back.
-// The two sides meet through named barriers (bar.arrive / bar.sync producer-consumer pairs): 1 = request
-// published, 2 = values ready, 3 = guess published.  While the contraction warps work the scalar warp evaluates
-// everything that does not need field values (the wave's exp / sincos, the next stage's partial sums, the
-// known part of the error ratio) and GUESSES THE NEXT POINT'S CELL (fp32, straight-line extrapolation along
-// the attempted step; at the end of an attempt from the accept/reject decision and the controller's new step
-// length).  A contraction lane starts fetching the guessed cell as soon as it is done with the current point
-// (eight 256-bit loads for the register half, one bulk asynchronous copy for the shared half), so the fetch
-// overlaps the scalar warp's work; a wrong guess only costs a blocking fetch.  The seven stage derivatives,
-// the step's start state and the per-particle bookkeeping live in shared memory, so the stage loop is rolled
-// (one copy of the right-hand side in the instruction stream) and nothing spills.
-#include <cstdlib>
-
+//     current cell, on chip (half in registers, half in a private conflict-free run of shared memory),
+//     re-fetched from the cell-major table only when the slot's cell changes.
+//
+// One right-hand-side evaluation ("round") is a two-sided pipeline instead of a ping-pong.  The three local
+// coordinates of a stage point do not become known at the same time: the FIRST (zeta / Z) is a state variable,
+// the SECOND (s / R) needs a square root, the LAST (theta / phi) an arctangent -- the longest dependent chain of
+// the scalar warp.  So the scalar warp publishes (wFIRST, wSECOND) as soon as it has them (barrier A) and goes on
+// with the arctangent, the wave terms and the cell index, while the contraction warps contract their 64
+// coefficients along FIRST and SECOND (60 of the 63 FMA) on the cell they hold and hand back the four plane
+// values P_0..P_3 of every quantity (barrier D); the scalar warp finishes with three FMA per quantity in wLAST.
+// The contraction therefore runs entirely in the shadow of the scalar warp's own chain.  The cell a contraction
+// lane holds at barrier A is the scalar warp's guess from the round before (fp32 straight-line extrapolation
+// along the attempted step, published at barrier G; after the accept/reject decision at barrier G2), fetched
+// while the scalar warp works; when the located cell turns out to differ (rare), the lane is told to redo the
+// contraction with the right cell (barrier D2).  The contraction warps also accumulate, one state component
+// each, the stage partial sums sum_j a_ij k_j and the error-estimate sums, off the scalar warp's critical path.
 #include "gc_device.cuh"
 
 namespace catapult {
 
-#ifndef CATAPULT_SPLIT_MINB_BOOZER
-#define CATAPULT_SPLIT_MINB_BOOZER 4
+#ifndef CATAPULT_MINB_BOOZER
+#define CATAPULT_MINB_BOOZER 4
 #endif
-#ifndef CATAPULT_SPLIT_MINB_CART
-#define CATAPULT_SPLIT_MINB_CART 2
+#ifndef CATAPULT_MINB_CART
+#define CATAPULT_MINB_CART 2
 #endif
 
 constexpr int MODE_ADAPTIVE = 0, MODE_SCRIPT = 1, MODE_STEP_ONCE = 2;
-
-#ifdef CATAPULT_PF_STATS
-__device__ unsigned long long g_blk[8];  // debugging aid: blocking fetches by request code
-extern "C" int catapult_debug_blocking(unsigned long long* out8) {
-  return cudaMemcpyFromSymbol(out8, g_blk, sizeof(g_blk)) != cudaSuccess;
-}
-#endif
 
 // Dormand-Prince 5(4) tableau for the rolled stage loop (row i = coefficients of the state fed to stage
 // i+2; the last row is b: the 7th stage is evaluated at the new state).  PAPER.md:61, ref [10].
@@ -55,39 +47,46 @@ __constant__ double DP_A[6][6] = {
 __constant__ double DP_C[6] = {1.0 / 5.0, 3.0 / 10.0, 4.0 / 5.0, 8.0 / 9.0, 1.0, 1.0};
 __constant__ double DP_E[7] = {71.0 / 57600.0, 0.0, -71.0 / 16695.0, 71.0 / 1920.0, -17253.0 / 339200.0,
                                22.0 / 525.0, -1.0 / 40.0};
+// Where along the attempted step the next evaluation point lies, relative to this one, in units of
+// (this point - start of the attempt): (c_next - c_this)/c_this for c = 1/5, 3/10, 4/5, 8/9, 1; after the last
+// point (the new state) the first point of the next attempt is guessed a fifth of a step further on.
+__constant__ float NEXT_POINT_RATIO[6] = {0.5f, 5.0f / 3.0f, 1.0f / 9.0f, 0.125f, 0.0f, 0.2f};
 
 template <int MODEL>
-struct SplitTraits {
+struct TraceTraits {
   static constexpr bool CART = (MODEL == MODEL_CART);
   static constexpr int NQ = CART ? CATAPULT_NQUANT_CYL : CATAPULT_NQUANT_BOOZER;
   static constexpr int NT = 32 * (NQ + 1);   // threads per block
   static constexpr int NCT = 32 * NQ;        // contraction threads per block
-  static constexpr int MINB = CART ? CATAPULT_SPLIT_MINB_CART : CATAPULT_SPLIT_MINB_BOOZER;
-  // A contraction thread keeps the first 32 stored coefficients of its (cell, quantity) block (the rows j = 0, 1
-  // of every slab, gc_device.cuh coef_row_pos) in registers and the other 32 in a private run of shared
-  // memory: 256 bytes + 16 bytes of padding, so that the 8 lanes of a quarter warp reading 16 bytes each at
-  // the same offset of their runs hit 8 different 16-byte bank groups.
+  static constexpr int MINB = CART ? CATAPULT_MINB_CART : CATAPULT_MINB_BOOZER;
+  // A contraction thread keeps the first 32 stored coefficients of its (cell, quantity) block (LAST-power 0, 1:
+  // gc_device.cuh) in registers and the other 32 in a private run of shared memory: 256 bytes + 16 bytes of
+  // padding, so that the 8 lanes of a quarter warp reading 16 bytes each at the same offset of their runs hit 8
+  // different 16-byte bank groups.
   static constexpr int STRIP = 272;
   // shared-memory layout (bytes)
-  static constexpr size_t OFF_COEF = 0;                              // [NCT] runs of STRIP bytes
-  static constexpr size_t OFF_MBAR = OFF_COEF + (size_t)STRIP * NCT;  // uint64 [NCT]: one mbarrier per thread
-  static constexpr size_t OFF_KS = OFF_MBAR + 8 * NCT;               // double [7][4][32]
-  static constexpr size_t OFF_W = OFF_KS + 7 * 4 * 32 * 8;           // double [3][32]
-  static constexpr size_t OFF_FV = OFF_W + 3 * 32 * 8;               // double [NQ][32]
-  static constexpr size_t OFF_REQ = OFF_FV + (size_t)NQ * 32 * 8;    // int2   [32]: code, flat cell index
-  static constexpr size_t OFF_POS = OFF_REQ + 32 * 8;                // float  [2][3][32]: last point, start point (cell units)
-  static constexpr size_t OFF_GUESS = OFF_POS + 2 * 3 * 32 * 4;      // int    [2][32]: guessed cell of the next point, by round parity
-  static constexpr size_t OFF_ERR = OFF_GUESS + 2 * 32 * 4;               // double [12][32]: known part of the error ratio; wave terms
-  static constexpr size_t OFF_Y = OFF_ERR + 12 * 32 * 8;               // double [9][32]: state y at the start of the step, dt, stage partial sums
-  static constexpr size_t OFF_COLD = OFF_Y + 9 * 32 * 8;                   // per-lane bookkeeping: 5 x int64[32] + 8 x int32[32]
-  static constexpr size_t SMEM_BYTES = OFF_COLD + 5 * 256 + 8 * 128;
+  static constexpr size_t OFF_COEF = 0;                               // [NCT] runs of STRIP bytes
+  static constexpr size_t OFF_MBAR = OFF_COEF + (size_t)STRIP * NCT;   // uint64 [NCT]: one mbarrier per thread
+  static constexpr size_t OFF_PART = OFF_MBAR + 8 * NCT;              // double2 [NQ][2][32]: plane values P_0..P_3
+  static constexpr size_t OFF_KS = OFF_PART + (size_t)NQ * 2 * 32 * 16;  // double [7][4][32]: stage derivatives
+  static constexpr size_t OFF_W = OFF_KS + 7 * 4 * 32 * 8;            // double [2][32]: wFIRST, wSECOND
+  static constexpr size_t OFF_P = OFF_W + 2 * 32 * 8;                 // double [4][32]: stage partial sums
+  static constexpr size_t OFF_ERR = OFF_P + 4 * 32 * 8;               // double [8][32]: error sums, 1/denominators
+  static constexpr size_t OFF_Y = OFF_ERR + 8 * 32 * 8;               // double [6][32]: y at the step's start, h, dt
+  static constexpr size_t OFF_G = OFF_Y + 6 * 32 * 8;                 // int2 [2][32]: (redo cell, next cell) by round parity
+  static constexpr size_t OFF_G2 = OFF_G + 2 * 32 * 8;                // int [32]: next cell after the accept/reject decision
+  static constexpr size_t OFF_REQ = OFF_G2 + 32 * 4;                  // int [32]: request word
+  static constexpr size_t OFF_BASE = OFF_REQ + 32 * 4;                // float [3][32]: start point of the attempt (cell units)
+  static constexpr size_t OFF_COLD = OFF_BASE + 3 * 32 * 4;           // per-lane bookkeeping: 7 x int64[32] + 8 x int32[32]
+  static constexpr size_t SMEM_BYTES = OFF_COLD + 7 * 256 + 8 * 128;
 };
 
-// Request of a slot: one word (what to evaluate: a stage point 0..5 of an attempted step, a start point, or
-// nothing; whether the kernel ends) + the flat cell index, and the local coordinates w[3].  The guess of the
-// NEXT point's cell travels separately (OFF_GUESS, barrier 3).
-constexpr int REQ_NONE = -1, REQ_START = 6;
-constexpr int CTL_PLAIN = 0, CTL_QUIT = 2;
+// Request word of a slot: bit 0 = the slot takes part in this round, bits 1-3 = kind of round (0..5: stage
+// point of an attempted step; 6: a start point), bit 4 = the kernel ends, bit 6 = parity of the round.
+constexpr int KIND_START = 6;
+constexpr int REQ_QUIT = 1 << 4;
+// named barriers (0 is __syncthreads')
+constexpr int BAR_A = 1, BAR_D = 2, BAR_G = 3 /* and 4: by round parity */, BAR_D2 = 5, BAR_G2 = 6;
 
 __device__ __forceinline__ void bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
@@ -123,8 +122,8 @@ __device__ __forceinline__ void mbar_wait(unsigned mbar, unsigned parity) {
   } while (!done);
 }
 
-// the 64 bytes of one slab's two shared rows (j = 2: v[0..3], j = 3: v[4..7]) as one batch of loads
-__device__ __forceinline__ void lds_slab(unsigned addr, double (&v)[8]) {
+// two rows (64 contiguous bytes) of the shared half as one batch of loads
+__device__ __forceinline__ void lds_rows2(unsigned addr, double (&v)[8]) {
   asm volatile(
       "ld.shared.v2.f64 {%0,%1}, [%8];\n\t"
       "ld.shared.v2.f64 {%2,%3}, [%8+16];\n\t"
@@ -135,12 +134,148 @@ __device__ __forceinline__ void lds_slab(unsigned addr, double (&v)[8]) {
       : "memory");
 }
 
-// ---- contraction warps -----------------------------------------------------------------------------
-// Where along the attempted step the next evaluation point lies, relative to this one, in units of
-// (this point - start of the attempt): (c_next - c_this)/c_this for c = 1/5, 3/10, 4/5, 8/9, 1.
-__constant__ float NEXT_POINT_RATIO[8] = {0.5f, 5.0f / 3.0f, 1.0f / 9.0f, 0.125f, 0.0f, 0.0f, 0.0f, 0.0f};
-__device__ __forceinline__ float next_point_ratio(int r) { return NEXT_POINT_RATIO[r & 7]; }
+// ---- contraction warps -----------------------------------------------------------------------------------------
+template <int MODEL>
+__device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned char* smem, int q, int lane) {
+  using TT = TraceTraits<MODEL>;
+  constexpr int NQ = TT::NQ, NT = TT::NT;
+  const unsigned FULL = 0xffffffffu;
+  const double* __restrict__ table = tc.f.table;
+  double reg[32];  // rows (a, b), a = 0, 1: reg[(a*4 + b)*4 + c]
+  unsigned char* strip = smem + TT::OFF_COEF + (size_t)(q * 32 + lane) * TT::STRIP;  // rows a = 2, 3
+  const unsigned strip_s = smem_u32(strip);
+  const unsigned mbar = smem_u32(smem + TT::OFF_MBAR) + 8u * (q * 32 + lane);
+  const double* wbuf = reinterpret_cast<const double*>(smem + TT::OFF_W);
+  double2* part = reinterpret_cast<double2*>(smem + TT::OFF_PART) + (q * 2) * 32 + lane;
+  const volatile int* reqbuf = reinterpret_cast<const volatile int*>(smem + TT::OFF_REQ);
+  const volatile long long* gbuf = reinterpret_cast<const volatile long long*>(smem + TT::OFF_G);
+  const volatile int* g2buf = reinterpret_cast<const volatile int*>(smem + TT::OFF_G2);
+  // stage sums: warp q < 4 owns state component q
+  const double* ks = reinterpret_cast<const double*>(smem + TT::OFF_KS) + (q & 3) * 32 + lane;  // k_j at ks[j*128]
+  double* pbuf = reinterpret_cast<double*>(smem + TT::OFF_P) + (q & 3) * 32 + lane;
+  double* errbuf = reinterpret_cast<double*>(smem + TT::OFF_ERR) + (q & 3) * 32 + lane;
+  const double* ysm = reinterpret_cast<const double*>(smem + TT::OFF_Y) + lane;
+  int cached = -1;
+  unsigned phase = 0;    // parity of the mbarrier phase the next wait is for
+  bool pending = false;  // a bulk copy into the strip is in flight
+  mbar_init(mbar, 1);
 
+  auto wait_strip = [&]() {
+    if (pending) {
+      mbar_wait(mbar, phase);
+      phase ^= 1u;
+      pending = false;
+    }
+  };
+  // a cell's 512 contiguous bytes of this lane's quantity: the first half lands in its final registers (eight
+  // 256-bit loads), the second half goes global -> shared as ONE bulk asynchronous copy.  Nothing waits here.
+  auto issue_loads = [&](int c) {
+    const double* src = table + ((long long)c * NQ + q) * 64;
+#pragma unroll
+    for (int e = 0; e < 32; e += 4) ldg_f64x4(src + e, reg[e], reg[e + 1], reg[e + 2], reg[e + 3]);
+    wait_strip();  // an earlier fetch may still be landing in the strip: let it finish first
+    mbar_expect_tx(mbar, 256);
+    bulk_g2s(strip_s, src + 32, 256, mbar);
+    pending = true;
+  };
+  // P_a = sum_bc C[a][b][c] wS^b wF^c for a = 0..3 (horner_plane of gc_device.cuh: same operations, same order;
+  // the shared half comes two rows at a time, rows b = 2, 3 of a plane before its rows b = 0, 1)
+  auto contract = [&](double wF, double wS) {
+    double v[8];
+    lds_rows2(strip_s + 64, v);  // plane 2, rows 2, 3
+    double P[2];
+#pragma unroll
+    for (int a = 0; a < 2; ++a) {
+      double row[4];
+#pragma unroll
+      for (int b = 0; b < 4; ++b) row[b] = reg[(a * 4 + b) * 4 + 3];
+#pragma unroll
+      for (int c = 2; c >= 0; --c)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) row[b] = fma(row[b], wF, reg[(a * 4 + b) * 4 + c]);
+      P[a] = horner_row(row[0], row[1], row[2], row[3], wS);
+    }
+    part[0] = make_double2(P[0], P[1]);
+#pragma unroll
+    for (int a = 0; a < 2; ++a) {
+      const double r3 = horner_row(v[4], v[5], v[6], v[7], wF);
+      const double r2 = horner_row(v[0], v[1], v[2], v[3], wF);
+      lds_rows2(strip_s + 128 * a, v);  // rows 0, 1 of this plane
+      double acc = fma(r3, wS, r2);
+      const double r1 = horner_row(v[4], v[5], v[6], v[7], wF);
+      const double r0 = horner_row(v[0], v[1], v[2], v[3], wF);
+      if (a == 0) lds_rows2(strip_s + 128 + 64, v);  // plane 3, rows 2, 3
+      acc = fma(acc, wS, r1);
+      P[a] = fma(acc, wS, r0);
+    }
+    part[32] = make_double2(P[0], P[1]);
+  };
+
+  for (;;) {
+    bar_sync(BAR_A, NT);
+    const int rq = reqbuf[lane];
+    if (rq & REQ_QUIT) break;  // block-uniform
+    const bool active = rq & 1;
+    const int kind = (rq >> 1) & 7;  // block-uniform
+    const int rpar = (rq >> 6) & 1;
+    const double wF = wbuf[lane], wS = wbuf[32 + lane];
+    if (active) {
+      wait_strip();
+      contract(wF, wS);
+    }
+    // ---- stage algebra of state component q: what the next round's stage state needs of the
+    // derivatives known so far; in the last round of an attempt everything of Eq. 4 that does not
+    // need the last derivative: c = (1,1,1,v_total), state and derivative at the start of the step
+    if (q < 4 && kind < KIND_START) {
+      if (kind < 5) {
+        double p = 0.0;
+        for (int j = 0; j <= kind; ++j) p = fma(DP_A[kind + 1][j], ks[j * 128], p);
+        pbuf[0] = p;
+      } else {
+        double e = 0.0;
+#pragma unroll
+        for (int j = 0; j < 6; ++j)
+          if (j != 1) e = fma(DP_E[j], ks[j * 128], e);
+        errbuf[0] = e;
+        const double sc = (q == 3) ? tc.atol * tc.vtot : tc.atol;
+        const double ah = fabs(ysm[4 * 32]);
+        errbuf[4 * 32] = fm::rcp(fma(tc.rtol, fma(ah, fabs(ks[0]), fabs(ysm[q * 32])), sc));
+      }
+    }
+    __syncwarp();
+    bar_arrive(BAR_D, NT);
+    // ---- the scalar warp has located the point: a wrong cell is redone; then the guessed cell of the next
+    // point is fetched while the scalar warp works on
+    bar_sync(BAR_G + rpar, NT);
+    const long long g = gbuf[rpar * 32 + lane];
+    const int redo_cell = (int)g, next_cell = (int)(g >> 32);
+    const bool redo = active && redo_cell >= 0;
+    if (__any_sync(FULL, redo)) {  // the same answer in every warp of the block
+      if (redo) {
+        issue_loads(redo_cell);
+        cached = redo_cell;
+        wait_strip();
+        contract(wF, wS);
+      }
+      __syncwarp();
+      bar_arrive(BAR_D2, NT);
+    }
+    if (active && next_cell >= 0 && next_cell != cached) {
+      issue_loads(next_cell);
+      cached = next_cell;
+    }
+    if (kind == 5) {  // end of an attempt: the first point of the next one depends on the accept/reject decision
+      bar_sync(BAR_G2, NT);
+      const int t2 = g2buf[lane];
+      if (active && t2 >= 0 && t2 != cached) {
+        issue_loads(t2);
+        cached = t2;
+      }
+    }
+  }
+}
+
+// ---- scalar warp ---------------------------------------------------------------------------------------------
 // cell of the point pos + ratio (pos - base), all in cell units (fp32: this is only a guess).  Periodic
 // dimensions: both points lie in [0, k), so the short way round differs from the plain difference by at most k.
 template <int MODEL>
@@ -159,157 +294,34 @@ __device__ __forceinline__ int guess_cell(const FieldConst& f, const float pos[3
   return flat_cell(f, ni[0], ni[1], ni[2]);
 }
 
-template <int MODEL>
-__device__ __forceinline__ void contraction_warp(const FieldConst& f, unsigned char* smem, int q, int lane,
-                                                 unsigned long long* counters) {
-  using ST = SplitTraits<MODEL>;
-  constexpr int NQ = ST::NQ, NT = ST::NT;
-  const double* __restrict__ table = f.table;
-  double reg[32];
-  unsigned char* strip = smem + ST::OFF_COEF + (size_t)(q * 32 + lane) * ST::STRIP;
-  const unsigned strip_s = smem_u32(strip);
-  const unsigned mbar = smem_u32(smem + ST::OFF_MBAR) + 8u * (q * 32 + lane);
-  const double* wbuf = reinterpret_cast<const double*>(smem + ST::OFF_W);
-  double* fvbuf = reinterpret_cast<double*>(smem + ST::OFF_FV);
-  const volatile int2* reqbuf = reinterpret_cast<const volatile int2*>(smem + ST::OFF_REQ);
-  const volatile int* guessbuf = reinterpret_cast<const volatile int*>(smem + ST::OFF_GUESS);
-  int cached = -1;
-  unsigned phase = 0;    // parity of the mbarrier phase the next wait is for
-  bool pending = false;  // a bulk copy into the strip is in flight
-#ifdef CATAPULT_PF_STATS
-  unsigned long long n_block = 0, n_pref = 0;
-#endif
-  mbar_init(mbar, 1);
-
-  // a cell's 512 contiguous bytes of this lane's quantity: the second half goes global -> shared as ONE bulk
-  // asynchronous copy (no register staging, no per-16-byte requests), the first half lands in its final
-  // registers.  Nothing waits here.
-  auto wait_strip = [&]() {
-    if (pending) {
-      mbar_wait(mbar, phase);
-      phase ^= 1u;
-      pending = false;
-    }
-  };
-  auto issue_loads = [&](int c) {
-    const double* src = table + ((long long)c * NQ + q) * 64;
-    // the eight vector loads first (they are the slower half: one request per 32 bytes), then the bulk copy
-#pragma unroll
-    for (int e = 0; e < 32; e += 4) ldg_f64x4(src + e, reg[e], reg[e + 1], reg[e + 2], reg[e + 3]);
-    wait_strip();  // a wrong guess may still be landing in the strip: let it finish first
-    mbar_expect_tx(mbar, 256);
-    bulk_g2s(strip_s, src + 32, 256, mbar);
-    pending = true;
-  };
-  for (;;) {
-    bar_sync(1, NT);
-    const long long rq_raw = *reinterpret_cast<const volatile long long*>(reqbuf + lane);  // one 8-byte load
-    const int2 rq = make_int2((int)rq_raw, (int)(rq_raw >> 32));
-    const int ctl = (rq.x >> 3) & 7;                            // block-uniform
-    if (ctl == CTL_QUIT) break;
-    const int code = (rq.x & 7) == 7 ? REQ_NONE : (rq.x & 7);
-    // the local coordinates are loaded with the request, not after it has been looked at (one latency, not two)
-    const double w0 = wbuf[lane], w1 = wbuf[32 + lane], w2 = wbuf[64 + lane];
-    if (code >= 0) {
-      const int c = rq.y;
-      if (c != cached) {  // the guess missed (or there was none): one memory latency, paid by the whole block
-        issue_loads(c);
-        cached = c;
-#ifdef CATAPULT_PF_STATS
-        ++n_block;
-        if (q == 0) atomicAdd(&g_blk[code & 7], 1ULL);
-#endif
-      }
-      wait_strip();
-      // horner64 (gc_device.cuh), same operations in the same order, scheduled by hand: the register half U
-      // (8 independent rows) is worked while the first batch of the shared half is in flight; the shared
-      // half V comes slab by slab, each slab's two rows as ONE batch of four 16-byte loads issued as soon as
-      // the previous batch has been consumed
-      double v[8];
-      lds_slab(strip_s + 64 * 3, v);
-      double U;
-      {
-        double pr[4];
-#pragma unroll
-        for (int g = 0; g < 2; ++g) {  // slabs 3,2 then 1,0: four rows at a time, level by level
-          double a4[4];
-#pragma unroll
-          for (int r = 0; r < 4; ++r) a4[r] = fma(reg[(4 * (1 - g) + r) * 4 + 3], w2, reg[(4 * (1 - g) + r) * 4 + 2]);
-#pragma unroll
-          for (int r = 0; r < 4; ++r) a4[r] = fma(a4[r], w2, reg[(4 * (1 - g) + r) * 4 + 1]);
-#pragma unroll
-          for (int r = 0; r < 4; ++r) a4[r] = fma(a4[r], w2, reg[(4 * (1 - g) + r) * 4]);
-          pr[2 * (1 - g) + 1] = fma(a4[3], w1, a4[2]);  // stored row = i*2 + j
-          pr[2 * (1 - g)] = fma(a4[1], w1, a4[0]);
-        }
-        U = fma(fma(fma(pr[3], w0, pr[2]), w0, pr[1]), w0, pr[0]);
-      }
-      double V = 0.0;
-#pragma unroll
-      for (int i = 3; i >= 0; --i) {
-        const double row1 = fma(fma(fma(v[7], w2, v[6]), w2, v[5]), w2, v[4]);
-        const double row0 = fma(fma(fma(v[3], w2, v[2]), w2, v[1]), w2, v[0]);
-        if (i > 0) lds_slab(strip_s + 64 * (i - 1), v);
-        const double pair = fma(row1, w1, row0);
-        V = (i == 3) ? pair : fma(V, w0, pair);
-      }
-      const double total = fma(V, w1 * w1, U);
-      fvbuf[q * 32 + lane] = total;
-    }
-    __syncwarp();
-    bar_arrive(2, NT);
-    // ---- while the scalar warp works: it publishes its guess of the NEXT point's cell (barrier 3: in its
-    // overlap window inside an attempted step; right after the accept/reject decision at its end); start
-    // fetching that cell if it is not the one held.  A wrong guess costs what every cell change cost before
-    // (a blocking fetch next round); a right one hides the fetch entirely.
-    bar_sync(3, NT);
-    int target = guessbuf[((rq.x >> 6) & 1) * 32 + lane];  // double-buffered by round parity
-    if (code < 0 || target < 0) target = cached;
-    if (target != cached) {
-#ifdef CATAPULT_PF_STATS
-      ++n_pref;
-#endif
-      issue_loads(target);
-      cached = target;
-    }
+// (c + i s)^m for an integer m (block-uniform): cos and sin of m times the angle whose cosine and sine are c, s
+__device__ __forceinline__ void unit_power(int m, double c, double s, double& cm, double& sm) {
+  if (m == 1) {
+    cm = c;
+    sm = s;
+    return;
   }
-#ifdef CATAPULT_PF_STATS
-  if (counters && q == 0) {  // debugging aid: blocking / guessed fetches of quantity 0 in the two spare status counters
-    atomicAdd(counters + 4, n_block);
-    atomicAdd(counters + 5, n_pref);
+  double bc = c, bs = s;
+  cm = 1.0;
+  sm = 0.0;
+  for (unsigned k = (unsigned)(m < 0 ? -m : m); k; k >>= 1) {
+    if (k & 1u) {
+      const double t = fma(cm, bc, -sm * bs);
+      sm = fma(cm, bs, sm * bc);
+      cm = t;
+    }
+    const double t = fma(bc, bc, -bs * bs);
+    bs = 2.0 * bc * bs;
+    bc = t;
   }
-#else
-  (void)counters;
-#endif
+  if (m < 0) sm = -sm;
 }
 
-// ---- scalar warp: geometry before the field values are known ------------------------------------------
 struct EvalGeo {
-  double a, inva, ang;                 // Boozer: s, 1/s, theta;  Cartesian: R, 1/R, phi
-  double sn, cs, Phihat, dPhihat;      // wave terms (MODEL_BOOZER_SAW)
+  double a, inva;                  // Boozer: s, 1/s;  Cartesian: R, 1/R
+  double ca, sa;                   // cosine and sine of theta (phi): y0/a, y1/a
+  double sn, cs, Phihat, dPhihat;  // wave terms (MODEL_BOOZER_SAW)
 };
-
-template <int MODEL>
-__device__ __forceinline__ void eval_locate(const TraceConst& tc, const double y[4], int i[3], double w[3],
-                                            float pos[3], EvalGeo& g) {
-  const double r2 = fma(y[0], y[0], y[1] * y[1]);
-  fm::sqrt_rsqrt(r2, g.a, g.inva);
-  g.ang = fm::atan2(y[1], y[0]);
-  if (MODEL == MODEL_CART) locate3<false>(tc.f, g.a, y[2], g.ang, i, w, pos);
-  else locate3<true>(tc.f, g.a, g.ang, y[2], i, w, pos);
-}
-
-// everything of the right-hand side that does not need the interpolated field (overlaps the contraction)
-template <int MODEL>
-__device__ __forceinline__ void eval_wave(const TraceConst& tc, double t, const double y[4], EvalGeo& g) {
-  if (MODEL == MODEL_BOOZER_SAW) {
-    const double ds = g.a - tc.saw_s0;
-    g.Phihat = tc.saw_Phi0 * fm::exp(-ds * ds * tc.saw_invw2);
-    g.dPhihat = g.Phihat * (-2.0 * ds * tc.saw_invw2);
-    const double eta = fma((double)tc.saw_m, g.ang, fma(-(double)tc.saw_n, y[2], tc.saw_omega * t));
-    fm::sincos(eta, g.sn, g.cs);
-  }
-}
 
 // DESIGN.md R1-R3 with the interpolated values fv
 template <int MODEL>
@@ -317,7 +329,7 @@ __device__ __forceinline__ void eval_physics(const TraceConst& tc, const double 
                                              const double* fv, double dy[4], double& modB, double& level) {
   const FieldConst& f = tc.f;
   if (MODEL == MODEL_CART) {
-    const double cph = y[0] * g.inva, sph = y[1] * g.inva;
+    const double cph = g.ca, sph = g.sa;
     const double BR = fv[0], Bp = fv[1], BZ = fv[2], gR = fv[3], gp = fv[4], gZ = fv[5];
     const double Bx = BR * cph - Bp * sph, By = BR * sph + Bp * cph, Bz = BZ;
     const double gx = gR * cph - gp * sph, gy = gR * sph + gp * cph, gz = gZ;
@@ -335,7 +347,7 @@ __device__ __forceinline__ void eval_physics(const TraceConst& tc, const double 
     modB = B;
     level = fv[6];
   } else {
-    const double s = g.a, invs = g.inva;
+    const double s = g.a;
     const double B = fv[0], B_s = fv[1], B_th = fv[2], B_ze = fv[3];
     const double vpar = y[3];
     const double invB = fm::rcp(B);
@@ -368,10 +380,8 @@ __device__ __forceinline__ void eval_physics(const TraceConst& tc, const double 
       const double t2 = tc.q * fma(al_t, f.G, fma(al_th * f.G, Phi_psi, fma(iag, Phi_th, Phi_ze)));
       vdot = fma(-(B * f.invG * tc.invM), t1 + t2, vpar * invB * fma(B_th, Phi_psi, -B_psi * Phi_th));
     }
-    const double c = (s > 0.0) ? y[0] * invs : 1.0;
-    const double sn_ = y[1] * invs;
-    dy[0] = fma(sdot, c, -thdot * y[1]);
-    dy[1] = fma(sdot, sn_, thdot * y[0]);
+    dy[0] = fma(sdot, g.ca, -thdot * y[1]);
+    dy[1] = fma(sdot, g.sa, thdot * y[0]);
     dy[2] = vBG;
     dy[3] = vdot;
     modB = B;
@@ -379,131 +389,146 @@ __device__ __forceinline__ void eval_physics(const TraceConst& tc, const double 
   }
 }
 
-// sum_{j < NJ} a[NJ][j] k_j: the part of stage state NJ + 2 (row NJ of DP_A) that is known before k_NJ is
-template <int NJ>
-__device__ __forceinline__ void stage_partial(const double* ks, double* P) {  // P: shared, stride 32
-#pragma unroll
-  for (int c = 0; c < 4; ++c) {
-    double k[NJ];
-#pragma unroll
-    for (int j = 0; j < NJ; ++j) k[j] = ks[(j * 4 + c) * 32];  // the loads of a component first, then its sum
-    double p = 0.0;
-#pragma unroll
-    for (int j = 0; j < NJ; ++j) p = fma(DP_A[NJ][j], k[j], p);
-    P[c * 32] = p;
-  }
-}
+struct ScalarRegs {   // what the scalar warp carries from round to round besides the particle state
+  int rpar;           // parity of the round (the guess buffer and its barrier are double-buffered by it)
+  int held;           // the cell this slot's contraction lanes hold (or are fetching)
+  unsigned n_load;    // cells fetched for this slot ...
+  unsigned n_block;   // ... of which after the point had been located (the guess missed)
+};
 
-// One lock-step evaluation round of the scalar warp, in two halves.  eval_publish: lanes with code >= 0 hand
-// (cell indices, w) of the point (t, y) to the contraction warps; the others publish REQ_NONE.  eval_collect:
-// picks up the interpolated values and finishes the right-hand side.  Between the two the caller may do
-// anything that does not need field values (it overlaps the contraction).  All 32 lanes must call both.
+// One lock-step right-hand-side evaluation of the scalar warp at the point (tr, X): see the top of this file.
+// Lanes with act = false publish a request nobody serves.  ratio >= 0: the next point is expected at
+// X + ratio (X - start of the attempt) and its cell is fetched ahead.  All 32 lanes must call this.
 template <int MODEL>
-__device__ __forceinline__ void eval_publish(const TraceConst& tc, unsigned char* smem, int lane, int code, int ctl,
-                                             int& rpar, double t, const double y[4], EvalGeo& g, float pos[3]) {
-  using ST = SplitTraits<MODEL>;
-  double* wbuf = reinterpret_cast<double*>(smem + ST::OFF_W);
-  int2* reqbuf = reinterpret_cast<int2*>(smem + ST::OFF_REQ);
-  float* posbuf = reinterpret_cast<float*>(smem + ST::OFF_POS);
-  int i[3];
-  double w[3];
-  eval_locate<MODEL>(tc, y, i, w, pos, g);
-  const int cell = flat_cell(tc.f, i[0], i[1], i[2]);
-  wbuf[lane] = w[0];
-  wbuf[32 + lane] = w[1];
-  wbuf[64 + lane] = w[2];
-  rpar ^= 1;  // round parity: selects the guess buffer of this round
-  reqbuf[lane] = make_int2((code < 0 ? 7 : code) | (ctl << 3) | (rpar << 6), cell);  // one word: what to do + what follows
-#pragma unroll
-  for (int d = 0; d < 3; ++d) posbuf[d * 32 + lane] = pos[d];
-  __syncwarp();
-  bar_arrive(1, ST::NT);
-  eval_wave<MODEL>(tc, t, y, g);
-}
-
-// the scalar warp's guess of the next evaluation point's cell (-1: none), handed over through barrier 3
-template <int MODEL>
-__device__ __forceinline__ void publish_guess(unsigned char* smem, int lane, int rpar, int target) {
-  using ST = SplitTraits<MODEL>;
-  reinterpret_cast<volatile int*>(smem + ST::OFF_GUESS)[rpar * 32 + lane] = target;
-  __syncwarp();
-  bar_arrive(3, ST::NT);
-}
-
-template <int MODEL>
-__device__ __forceinline__ void eval_collect(const TraceConst& tc, unsigned char* smem, int lane, const double y[4],
-                                             double mu, EvalGeo& g, double dy[4], double& modB, double& level) {
-  using ST = SplitTraits<MODEL>;
-  const double* fvbuf = reinterpret_cast<const double*>(smem + ST::OFF_FV);
-  // The wave terms cross the barrier through shared memory: stores cannot move across a barrier, so the
-  // arithmetic that produces them stays in the overlap window (ptxas otherwise sinks it below the barrier, onto
-  // the critical path, to save the registers they would occupy across it).
-  double* wavebuf = reinterpret_cast<double*>(smem + ST::OFF_ERR) + 8 * 32 + lane;
-  if (MODEL == MODEL_BOOZER_SAW) {
-    wavebuf[0] = g.sn;
-    wavebuf[32] = g.cs;
-    wavebuf[64] = g.Phihat;
-    wavebuf[96] = g.dPhihat;
-  }
-  bar_sync(2, ST::NT);
-  double fv[ST::NQ];
-#pragma unroll
-  for (int q = 0; q < ST::NQ; ++q) fv[q] = fvbuf[q * 32 + lane];
-  if (MODEL == MODEL_BOOZER_SAW) {
-    g.sn = wavebuf[0];
-    g.cs = wavebuf[32];
-    g.Phihat = wavebuf[64];
-    g.dPhihat = wavebuf[96];
-  }
-  eval_physics<MODEL>(tc, y, mu, g, fv, dy, modB, level);
-}
-
-template <int MODEL>
-__device__ __forceinline__ void eval_round(const TraceConst& tc, unsigned char* smem, int lane, int code, int& rpar,
-                                           double t, const double y[4], double mu, double dy[4], double& modB,
-                                           double& level) {
-  using ST = SplitTraits<MODEL>;
+__device__ __forceinline__ void scalar_round(const TraceConst& tc, unsigned char* smem, int lane, bool act, int kind,
+                                             ScalarRegs& sr, double tr, const double X[4], double mu, float ratio,
+                                             float pos[3], double dy[4], double& modB, double& level) {
+  using TT = TraceTraits<MODEL>;
+  constexpr bool BZ = (MODEL != MODEL_CART);
+  using AX = AxisRoles<BZ>;
+  constexpr int NT = TT::NT;
+  const unsigned FULL = 0xffffffffu;
+  const FieldConst& f = tc.f;
+  double* wbuf = reinterpret_cast<double*>(smem + TT::OFF_W);
+  int* reqbuf = reinterpret_cast<int*>(smem + TT::OFF_REQ);
+  int2* gbuf = reinterpret_cast<int2*>(smem + TT::OFF_G);
+  const float* basebuf = reinterpret_cast<const float*>(smem + TT::OFF_BASE);
   EvalGeo g;
-  float pos[3];
-  eval_publish<MODEL>(tc, smem, lane, code, CTL_PLAIN, rpar, t, y, g, pos);
-  if (code >= 0) {  // a start point: the next attempted step is extrapolated from here
-    float* basebuf = reinterpret_cast<float*>(smem + ST::OFF_POS) + 96;
-#pragma unroll
-    for (int d = 0; d < 3; ++d) basebuf[d * 32 + lane] = pos[d];
+  int ci[3];
+  double wF, wS, wL;
+  // ---- the two coordinates that are known early
+  const double r2 = fma(X[0], X[0], X[1] * X[1]);
+  fm::sqrt_rsqrt(r2, g.a, g.inva);
+  {
+    double xr = X[2] - f.lo[AX::FIRST];
+    if (BZ) xr = wrap_periodic(xr, f.span[AX::FIRST], f.invspan[AX::FIRST]);
+    ci[AX::FIRST] = cell_and_w(xr, f.invh[AX::FIRST], f.k[AX::FIRST], wF, pos[AX::FIRST]);
   }
-  publish_guess<MODEL>(smem, lane, rpar, -1);
-  eval_collect<MODEL>(tc, smem, lane, y, mu, g, dy, modB, level);
+  ci[AX::SECOND] = cell_and_w(g.a - f.lo[AX::SECOND], f.invh[AX::SECOND], f.k[AX::SECOND], wS, pos[AX::SECOND]);
+  wbuf[lane] = wF;
+  wbuf[32 + lane] = wS;
+  sr.rpar ^= 1;
+  reqbuf[lane] = (act ? 1 : 0) | (kind << 1) | (sr.rpar << 6);
+  __syncwarp();
+  bar_arrive(BAR_A, NT);
+  // ---- in the shadow of the arctangent: unit vector, wave terms
+  g.ca = (BZ && !(g.a > 0.0)) ? 1.0 : X[0] * g.inva;
+  g.sa = X[1] * g.inva;
+  if (MODEL == MODEL_BOOZER_SAW) {
+    const double ds = g.a - tc.saw_s0;
+    g.Phihat = tc.saw_Phi0 * fm::exp(-ds * ds * tc.saw_invw2);
+    g.dPhihat = g.Phihat * (-2.0 * ds * tc.saw_invw2);
+    // sin / cos of m theta - n zeta + omega t by the addition theorem: cos / sin of theta are y0/s, y1/s, so the
+    // wave does not wait for the arctangent
+    const double beta = fma(-(double)tc.saw_n, X[2], tc.saw_omega * tr);
+    double sb, cb, cm, sm;
+    fm::sincos(beta, sb, cb);
+    unit_power(tc.saw_m, g.ca, g.sa, cm, sm);
+    g.sn = fma(sm, cb, cm * sb);
+    g.cs = fma(cm, cb, -sm * sb);
+  }
+  // ---- the last coordinate and the cell
+  {
+    const double ang = fm::atan2(X[1], X[0]);
+    const double xr = wrap_periodic(ang - f.lo[AX::LAST], f.span[AX::LAST], f.invspan[AX::LAST]);
+    ci[AX::LAST] = cell_and_w(xr, f.invh[AX::LAST], f.k[AX::LAST], wL, pos[AX::LAST]);
+  }
+  const int cell = flat_cell(f, ci[0], ci[1], ci[2]);
+  const bool bad = act && cell != sr.held;  // the contraction ran on another cell's coefficients: redo
+  int target = -1;
+  if (act && ratio >= 0.f) {
+    const float base[3] = {basebuf[lane], basebuf[32 + lane], basebuf[64 + lane]};
+    target = guess_cell<MODEL>(f, pos, base, ratio);
+  }
+  gbuf[sr.rpar * 32 + lane] = make_int2(bad ? cell : -1, target);
+  if (act) {
+    const int now = bad ? cell : sr.held;
+    const int next = target >= 0 ? target : now;
+    sr.n_block += bad;
+    sr.n_load += (unsigned)bad + (unsigned)(next != now);
+    sr.held = next;
+  }
+  __syncwarp();
+  bar_arrive(BAR_G + sr.rpar, NT);
+  const bool anybad = __any_sync(FULL, bad);
+  bar_sync(BAR_D, NT);
+  if (anybad) bar_sync(BAR_D2, NT);
+  // ---- plane values -> field values (the last three FMA of horner64), then the right-hand side
+  const double2* part = reinterpret_cast<const double2*>(smem + TT::OFF_PART) + lane;
+  double fv[TT::NQ];
+#pragma unroll
+  for (int q = 0; q < TT::NQ; ++q) {
+    const double2 p01 = part[(q * 2) * 32], p23 = part[(q * 2 + 1) * 32];
+    fv[q] = horner_row(p01.x, p01.y, p23.x, p23.y, wL);
+  }
+  eval_physics<MODEL>(tc, X, mu, g, fv, dy, modB, level);
 }
 
 template <int MODEL, int MODE>
-__global__ void __launch_bounds__(SplitTraits<MODEL>::NT, SplitTraits<MODEL>::MINB)
+__global__ void __launch_bounds__(TraceTraits<MODEL>::NT, TraceTraits<MODEL>::MINB)
 trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ TraceArgs a) {
-  using ST = SplitTraits<MODEL>;
+  using TT = TraceTraits<MODEL>;
   extern __shared__ __align__(16) unsigned char smem[];
   const int lane = threadIdx.x & 31;
   const int warp = threadIdx.x >> 5;
-  if (warp < ST::NQ) {
-    contraction_warp<MODEL>(tc.f, smem, warp, lane, a.counters);
+  if (warp < TT::NQ) {
+    contraction_warp<MODEL>(tc, smem, warp, lane);
     return;
   }
 
   // ---- scalar warp ------------------------------------------------------------------------------------
   const unsigned FULL = 0xffffffffu;
   const long long n = a.n;
-  double* ks = reinterpret_cast<double*>(smem + ST::OFF_KS) + lane;  // k_j component c at ks[(j*4+c)*32]
-  double t = 0.0, mu = 0.0;
-  double* ysm = reinterpret_cast<double*>(smem + ST::OFF_Y) + lane;  // y_c of the step's start at ysm[c * 32]
-  double& dt = ysm[4 * 32];
+  // DESIGN.md S3: default step lengths (Boozer: L = |G| / |B|(node 0), read from the device scalar the field
+  // build left; the cylindrical default is resolved on the host)
+  double dtmax = tc.dtmax, dt0 = tc.dt0;
+  if (!(dtmax > 0.0)) {
+    const double L = __ddiv_rn(fabs(tc.f.G), fabs(*tc.f.node0));
+    dtmax = __ddiv_rn(__dmul_rn(0.5 * 3.14159265358979323846, L), tc.vtot);
+    dt0 = dt0 > 0.0 ? dt0 : __dmul_rn(1e-3, dtmax);
+    dt0 = dt0 > dtmax ? dtmax : dt0;
+  }
+  double* ks = reinterpret_cast<double*>(smem + TT::OFF_KS) + lane;    // k_j component c at ks[(j*4+c)*32]
+  double* ysm = reinterpret_cast<double*>(smem + TT::OFF_Y) + lane;    // y_c of the step's start at ysm[c*32]
+  double& hsm = ysm[4 * 32];                                          // length of the attempted step
+  double& dt = ysm[5 * 32];                                           // the controller's step length
+  const double* pbuf = reinterpret_cast<const double*>(smem + TT::OFF_P) + lane;
+  const double* errbuf = reinterpret_cast<const double*>(smem + TT::OFF_ERR) + lane;  // [c]: sum, [4 + c]: 1/denominator
+  float* basebuf = reinterpret_cast<float*>(smem + TT::OFF_BASE) + lane;
+  int* g2buf = reinterpret_cast<int*>(smem + TT::OFF_G2);
   dt = 0.0;
-  // bookkeeping that is touched once per attempted step or once per particle lives in shared memory, not in
-  // registers (the compiler would spill it to local memory, whose reloads sat on the critical path)
-  long long* cold64 = reinterpret_cast<long long*>(smem + ST::OFF_COLD) + lane;
-  unsigned* cold32 = reinterpret_cast<unsigned*>(smem + ST::OFF_COLD + 5 * 256) + lane;
+  hsm = 0.0;
+  double t = 0.0, mu = 0.0;
+  // bookkeeping that is touched once per attempted step or once per particle lives in shared memory
+  long long* cold64 = reinterpret_cast<long long*>(smem + TT::OFF_COLD) + lane;
+  unsigned* cold32 = reinterpret_cast<unsigned*>(smem + TT::OFF_COLD + 7 * 256) + lane;
   long long& idx = cold64[0 * 32];
   long long& attempts_left = cold64[1 * 32];
   unsigned long long& c_acc = reinterpret_cast<unsigned long long&>(cold64[2 * 32]);
   unsigned long long& c_rej = reinterpret_cast<unsigned long long&>(cold64[3 * 32]);
   unsigned long long& c_eval = reinterpret_cast<unsigned long long&>(cold64[4 * 32]);
+  unsigned long long& c_load = reinterpret_cast<unsigned long long&>(cold64[5 * 32]);
+  unsigned long long& c_block = reinterpret_cast<unsigned long long&>(cold64[6 * 32]);
   unsigned& nacc = cold32[0 * 32];
   unsigned& nrej = cold32[1 * 32];
   int& consecutive = reinterpret_cast<int&>(cold32[2 * 32]);
@@ -511,13 +536,14 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
   unsigned* c_fin = cold32 + 4 * 32;  // c_fin[s] at c_fin[s * 32]
   idx = -1;
   attempts_left = 0;
-  c_acc = c_rej = c_eval = 0;
+  c_acc = c_rej = c_eval = c_load = c_block = 0;
   nacc = nrej = 0;
   consecutive = step = 0;
 #pragma unroll
   for (int j = 0; j < 4; ++j) c_fin[j * 32] = 0;
   bool active = false, exhausted = false;
-  int rpar = 0;  // parity of the evaluation round (the guess buffer is double-buffered by it)
+  ScalarRegs sr{0, -1, 0u, 0u};
+  unsigned long long rounds = 0;  // warp-uniform
 
   for (;;) {
     // ---- refill: lanes without a particle pull the next index (one atomic per warp) ------------------
@@ -558,7 +584,9 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
     if (__any_sync(FULL, fresh)) {
       // the start point's field values give mu and k1
       double dy0[4], B, level;
-      eval_round<MODEL>(tc, smem, lane, fresh ? REQ_START : REQ_NONE, rpar, t, y, 0.0, dy0, B, level);
+      float pos[3];
+      scalar_round<MODEL>(tc, smem, lane, fresh, KIND_START, sr, t, y, 0.0, -1.f, pos, dy0, B, level);
+      ++rounds;
       if (fresh) {
         ++c_eval;
         if (MODE != MODE_STEP_ONCE && a.resume) {
@@ -566,7 +594,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
           dt = a.dt_io[idx];
         } else {
           mu = (tc.vtot2 - x[3] * x[3]) / (2.0 * B);
-          dt = tc.dt0;
+          dt = dt0;
         }
         if (MODE != MODE_STEP_ONCE && !a.resume && is_lost<MODEL>(tc, level)) {
           // born outside: returned unchanged, t_stop = 0
@@ -588,17 +616,21 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
           active = true;
         }
       }
-      // k1 with the particle's own mu: the field values are those of the round above; only the physics
-      // is redone (mu enters linearly; the geometry is recomputed from y, cheap and rare)
-      if (__any_sync(FULL, fresh && active)) {
-        eval_round<MODEL>(tc, smem, lane, (fresh && active) ? REQ_START : REQ_NONE, rpar, t, y, mu, dy0, B, level);
-        if (fresh && active) {
+      // k1 with the particle's own mu (mu enters the right-hand side linearly; the round is simply repeated:
+      // once per particle)
+      const bool go = fresh && active;
+      if (__any_sync(FULL, go)) {
+        scalar_round<MODEL>(tc, smem, lane, go, KIND_START, sr, t, y, mu, -1.f, pos, dy0, B, level);
+        ++rounds;
+        if (go) {
           ++c_eval;
 #pragma unroll
           for (int c = 0; c < 4; ++c) {
             ks[c * 32] = dy0[c];
             ysm[c * 32] = y[c];
           }
+#pragma unroll
+          for (int d = 0; d < 3; ++d) basebuf[d * 32] = pos[d];  // the first attempt is extrapolated from here
           nacc = 0;
           nrej = 0;
           consecutive = 0;
@@ -632,74 +664,29 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
     }
     const bool stepping = active && finish < 0;
     if (__any_sync(FULL, stepping)) {
-      double ys[4], dy[4], B_, level = 0.0;
-      double* P = ysm + 5 * 32;  // sum_{j<st} a[st][j] k_j of the next stage, written in the overlap window
-      double* errbuf = reinterpret_cast<double*>(smem + ST::OFF_ERR) + lane;  // [c]: sum, [4 + c]: 1/denominator
+      double X[4], dy[4], B_, level = 0.0;
+      float pos[3];
+      hsm = h;
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        dy[c] = ks[c * 32];  // k1 (first-same-as-last, or the start point's derivative)
-        P[c * 32] = 0.0;
-      }
-      EvalGeo g;
-      // one stage point: its state, the request, and everything that overlaps the contraction
-      auto stage_publish = [&](int st) {
-        // stage state y + h sum_{j<=st} a[st][j] k_j (row 5 = b: the new state); the sum over j < st was
-        // accumulated while the previous contraction ran, the newest derivative enters last
-        const double ad = DP_A[st][st];
-#pragma unroll
-        for (int c = 0; c < 4; ++c) ys[c] = fma(h, fma(ad, dy[c], P[c * 32]), ysm[c * 32]);
-        float pos[3];
-        eval_publish<MODEL>(tc, smem, lane, stepping ? st : REQ_NONE, CTL_PLAIN, rpar, fma(DP_C[st], h, t), ys, g, pos);
-        // ---- overlaps the contraction ----
-        if (st < 5 || MODE == MODE_STEP_ONCE) {
-          // the next point's cell, guessed by straight-line extrapolation from the step's start point (fp32,
-          // cell units): the contraction warps start fetching it as soon as they are done with this point
-          int target = -1;
-          if (stepping && st < 5) {
-            const float* basebuf = reinterpret_cast<const float*>(smem + ST::OFF_POS) + 96;
-            const float base[3] = {basebuf[lane], basebuf[32 + lane], basebuf[64 + lane]};
-            target = guess_cell<MODEL>(tc.f, pos, base, next_point_ratio(st));
-          }
-          publish_guess<MODEL>(smem, lane, rpar, target);
-        }
-        if (st < 5) {
-          switch (st) {  // all the loads of a row first, then its sums (j ascending, as everywhere)
-            case 0: stage_partial<1>(ks, P); break;
-            case 1: stage_partial<2>(ks, P); break;
-            case 2: stage_partial<3>(ks, P); break;
-            case 3: stage_partial<4>(ks, P); break;
-            default: stage_partial<5>(ks, P); break;
-          }
-        } else {
-          // PAPER.md:85 Eq. 4, c = (1,1,1,v_total), state and derivative at the start of the
-          // step: everything of the error ratio that does not need the last derivative
-          const double ah = fabs(h);
-#pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            double e = 0.0;
-#pragma unroll
-            for (int j = 0; j < 6; ++j)
-              if (j != 1) e = fma(DP_E[j], ks[(j * 4 + c) * 32], e);
-            errbuf[c * 32] = e;
-            const double sc = (c == 3) ? tc.atol * tc.vtot : tc.atol;
-            errbuf[(4 + c) * 32] = fm::rcp(fma(tc.rtol, fma(ah, fabs(ks[c * 32]), fabs(ysm[c * 32])), sc));
-          }
-        }
-      };
-      // The loop is cut between the overlap window and the pick-up of the values, so that the critical part of a
-      // round (values -> physics -> next stage state -> locate -> request) is one straight-line block in which
-      // the compiler can interleave the short critical chain with the rest.
-      stage_publish(0);
+      for (int c = 0; c < 4; ++c) dy[c] = ks[c * 32];  // k1 (first-same-as-last, or the start point's derivative)
 #pragma unroll 1
-      for (int st = 0; st < 5; ++st) {
-        eval_collect<MODEL>(tc, smem, lane, ys, mu, g, dy, B_, level);
+      for (int r = 0; r < 6; ++r) {
+        // stage state y + h sum_{j<=r} a[r][j] k_j (row 5 = b: the new state); the sum over j < r was
+        // accumulated by the contraction warps during the previous round, the newest derivative enters last
+        const double ad = DP_A[r][r];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) ks[((st + 1) * 4 + c) * 32] = dy[c];
-        stage_publish(st + 1);
+        for (int c = 0; c < 4; ++c) {
+          const double Pc = r > 0 ? pbuf[c * 32] : 0.0;
+          X[c] = fma(h, fma(ad, dy[c], Pc), ysm[c * 32]);
+        }
+        const float ratio = (MODE == MODE_STEP_ONCE && r == 5) ? -1.f : NEXT_POINT_RATIO[r];
+        scalar_round<MODEL>(tc, smem, lane, stepping, r, sr, fma(DP_C[r], h, t), X, mu, ratio, pos, dy, B_, level);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) ks[((r + 1) * 4 + c) * 32] = dy[c];
       }
-      eval_collect<MODEL>(tc, smem, lane, ys, mu, g, dy, B_, level);
-#pragma unroll
-      for (int c = 0; c < 4; ++c) ks[(6 * 4 + c) * 32] = dy[c];
+      rounds += 6;
+      // PAPER.md:85 Eq. 4: the contraction warps left the sums over the first six derivatives and the
+      // reciprocal denominators
       double r = 0.0, chk = 0.0;
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
@@ -712,31 +699,31 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
       bool accepted = false;
       double dtn = h;
       if (MODE == MODE_SCRIPT) accepted = true;
-      else if (MODE == MODE_ADAPTIVE) dtn = controller(h, r, tc.dtmax, accepted);
-      if (MODE != MODE_STEP_ONCE) {
-        // the decision goes to the contraction warps at once, with the length of the next attempt over this
-        // one's: they guess the cell of its first point (a rejected step is retried from the start point)
-        double hn = h;
-        if (MODE == MODE_ADAPTIVE) {
-          const double tn = accepted ? (clamped ? tc.T : t + h) : t;
-          hn = fmin((accepted && clamped) ? dt : dtn, tc.T - tn);
-        }
-        // first point of the next attempt: end point + ratio (end - start); accepted: a fifth of the next
-        // step over this one beyond the end point, which becomes the new start point; rejected: the same,
-        // measured from the start point
-        const float fr = 0.2f * __fdividef((float)hn, (float)h);
+      else if (MODE == MODE_ADAPTIVE) dtn = controller(h, r, dtmax, accepted);
+      {
+        // the decision goes to the contraction warps at once: the cell of the next attempt's first point, a
+        // fifth of the next step length beyond the new start point (accepted: the end point; rejected: the old
+        // start point)
         int target = -1;
-        if (stepping) {
-          float* posbuf = reinterpret_cast<float*>(smem + ST::OFF_POS);
-          const float pe[3] = {posbuf[lane], posbuf[32 + lane], posbuf[64 + lane]};
-          const float base[3] = {posbuf[96 + lane], posbuf[128 + lane], posbuf[160 + lane]};
-          target = guess_cell<MODEL>(tc.f, pe, base, accepted ? fr : fr - 1.0f);
+        if (MODE != MODE_STEP_ONCE && stepping) {
+          double hn = h;
+          if (MODE == MODE_ADAPTIVE) {
+            const double tn = accepted ? (clamped ? tc.T : t + h) : t;
+            hn = fmin((accepted && clamped) ? dt : dtn, tc.T - tn);
+          }
+          const float fr = 0.2f * __fdividef((float)hn, (float)h);
+          const float base[3] = {basebuf[0], basebuf[32], basebuf[64]};
+          target = guess_cell<MODEL>(tc.f, pos, base, accepted ? fr : fr - 1.0f);
+          sr.n_load += (unsigned)(target != sr.held);
+          sr.held = target;
           if (accepted) {
 #pragma unroll
-            for (int d = 0; d < 3; ++d) posbuf[96 + d * 32 + lane] = pe[d];
+            for (int d = 0; d < 3; ++d) basebuf[d * 32] = pos[d];
           }
         }
-        publish_guess<MODEL>(smem, lane, rpar, target);
+        g2buf[lane] = target;
+        __syncwarp();
+        bar_arrive(BAR_G2, TT::NT);
       }
       if (stepping) {
         c_eval += 6;
@@ -746,7 +733,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
           ++step;
         } else if (MODE == MODE_STEP_ONCE) {
           double xn[4];
-          y_to_state<MODEL>(ys, xn);
+          y_to_state<MODEL>(X, xn);
 #pragma unroll
           for (int c = 0; c < 4; ++c) a.x_out[c * n + idx] = xn[c];
           a.script_r[idx] = r;
@@ -768,7 +755,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
             if (!clamped) dt = dtn;
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-              ysm[c * 32] = ys[c];
+              ysm[c * 32] = X[c];
               ks[c * 32] = dy[c];  // first-same-as-last
             }
             // DESIGN.md S5: loss first, then T
@@ -792,6 +779,9 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
       if (a.nrej) a.nrej[idx] = (a.resume ? a.nrej[idx] : 0u) + nrej;
       c_acc += nacc;
       c_rej += nrej;
+      c_load += sr.n_load;
+      c_block += sr.n_block;
+      sr.n_load = sr.n_block = 0;
       ++c_fin[finish * 32];
       active = false;
     }
@@ -799,86 +789,94 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
 
   // release the contraction warps
   {
-    reinterpret_cast<int2*>(smem + ST::OFF_REQ)[lane] = make_int2(7 | (CTL_QUIT << 3), 0);
+    reinterpret_cast<int*>(smem + TT::OFF_REQ)[lane] = REQ_QUIT;
     __syncwarp();
-    bar_arrive(1, ST::NT);
+    bar_arrive(BAR_A, TT::NT);
   }
 
   // ---- statistics: one atomic per warp per counter -----------------------------------------------------
   if (a.counters) {
-    unsigned long long v[7] = {c_acc, c_rej, c_fin[0], c_fin[32], c_fin[64], c_fin[96], c_eval};
+    unsigned long long v[CATAPULT_NCOUNTERS] = {c_acc,      c_rej,  c_fin[0],           c_fin[32],           c_fin[64],
+                                                c_fin[96],  c_eval, c_load + sr.n_load, c_block + sr.n_block, 0};
 #pragma unroll
-    for (int j = 0; j < 7; ++j) {
+    for (int j = 0; j < CATAPULT_NCOUNTERS - 1; ++j) {
       unsigned long long s = v[j];
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(FULL, s, o);
       if (lane == 0 && s) atomicAdd(a.counters + j, s);
     }
+    if (lane == 0 && rounds) atomicAdd(a.counters + CATAPULT_NCOUNTERS - 1, rounds);
   }
 }
 
 // ---- launchers ---------------------------------------------------------------------------------------------
+// Persistent grid: resident blocks per SM x SM count (or fewer when there are fewer particles than slots).  The
+// shape of a (model, mode) pair on a device is computed once and cached.
+struct LaunchShape {
+  int device = -1, resident = 0;
+};
+
 template <int MODEL, int MODE>
-static catapult_status split_shape(int64_t n, int* blocks, int* threads) {
-  using ST = SplitTraits<MODEL>;
-  int dev = 0, sms = 0, per_sm = 0;
+static catapult_status trace_shape(int64_t n, int* blocks, int* threads) {
+  using TT = TraceTraits<MODEL>;
+  static thread_local LaunchShape cache;
+  int dev = 0;
   CATAPULT_CUDA_TRY(cudaGetDevice(&dev));
-  CATAPULT_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  CATAPULT_CUDA_TRY(cudaFuncSetAttribute(trace_kernel<MODEL, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)ST::SMEM_BYTES));
-  CATAPULT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<MODEL, MODE>, ST::NT,
-                                                                  ST::SMEM_BYTES));
-  if (per_sm < 1) {
-    set_error("the tracer kernel does not fit on this device (registers / shared memory)");
-    return CATAPULT_ECUDA;
+  if (cache.device != dev) {
+    int sms = 0, per_sm = 0;
+    CATAPULT_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CATAPULT_CUDA_TRY(cudaFuncSetAttribute(trace_kernel<MODEL, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)TT::SMEM_BYTES));
+    CATAPULT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<MODEL, MODE>, TT::NT,
+                                                                    TT::SMEM_BYTES));
+    if (per_sm < 1) {
+      set_error("the tracer kernel does not fit on this device (registers / shared memory)");
+      return CATAPULT_ECUDA;
+    }
+    cache.device = dev;
+    cache.resident = sms * per_sm;  // a multiple of the SM count
   }
-  if (const char* e = getenv("CATAPULT_BLOCKS_PER_SM")) {  // experiments only
-    const int v = atoi(e);
-    if (v >= 1 && v < per_sm) per_sm = v;
-  }
-  const long long resident = (long long)sms * per_sm;  // persistent: a multiple of the SM count
   long long want = (n + 31) / 32;
   if (want < 1) want = 1;
-  *blocks = (int)(want < resident ? want : resident);
-  *threads = ST::NT;
+  *blocks = (int)(want < cache.resident ? want : cache.resident);
+  *threads = TT::NT;
   return CATAPULT_OK;
 }
 
 template <int MODEL, int MODE>
-static catapult_status split_launch(const TraceConst& tc, const TraceArgs& a, cudaStream_t s) {
-  using ST = SplitTraits<MODEL>;
+static catapult_status trace_launch(const TraceConst& tc, const TraceArgs& a, cudaStream_t s) {
+  using TT = TraceTraits<MODEL>;
   int blocks = 0, threads = 0;
-  catapult_status st = split_shape<MODEL, MODE>(a.n, &blocks, &threads);
+  catapult_status st = trace_shape<MODEL, MODE>(a.n, &blocks, &threads);
   if (st != CATAPULT_OK) return st;
-  trace_kernel<MODEL, MODE><<<blocks, threads, ST::SMEM_BYTES, s>>>(tc, a);
+  trace_kernel<MODEL, MODE><<<blocks, threads, TT::SMEM_BYTES, s>>>(tc, a);
   CATAPULT_CUDA_TRY(cudaGetLastError());
   return CATAPULT_OK;
 }
 
 template <int MODE>
-static catapult_status split_dispatch(const TraceConst& tc, const TraceArgs& a, int model, cudaStream_t s) {
+static catapult_status trace_dispatch(const TraceConst& tc, const TraceArgs& a, int model, cudaStream_t s) {
   if (a.n == 0) return CATAPULT_OK;
   switch (model) {
-    case MODEL_BOOZER_VAC: return split_launch<MODEL_BOOZER_VAC, MODE>(tc, a, s);
-    case MODEL_BOOZER_SAW: return split_launch<MODEL_BOOZER_SAW, MODE>(tc, a, s);
-    default: return split_launch<MODEL_CART, MODE>(tc, a, s);
+    case MODEL_BOOZER_VAC: return trace_launch<MODEL_BOOZER_VAC, MODE>(tc, a, s);
+    case MODEL_BOOZER_SAW: return trace_launch<MODEL_BOOZER_SAW, MODE>(tc, a, s);
+    default: return trace_launch<MODEL_CART, MODE>(tc, a, s);
   }
 }
 
 catapult_status launch_trace(const TraceConst& tc, const TraceArgs& a, int model, int mode, cudaStream_t s) {
   switch (mode) {
-    case MODE_ADAPTIVE: return split_dispatch<MODE_ADAPTIVE>(tc, a, model, s);
-    case MODE_SCRIPT: return split_dispatch<MODE_SCRIPT>(tc, a, model, s);
-    default: return split_dispatch<MODE_STEP_ONCE>(tc, a, model, s);
+    case MODE_ADAPTIVE: return trace_dispatch<MODE_ADAPTIVE>(tc, a, model, s);
+    case MODE_SCRIPT: return trace_dispatch<MODE_SCRIPT>(tc, a, model, s);
+    default: return trace_dispatch<MODE_STEP_ONCE>(tc, a, model, s);
   }
 }
 
-
 catapult_status trace_launch_shape(int model, int64_t n, int* blocks, int* threads) {
   switch (model) {
-    case MODEL_BOOZER_VAC: return split_shape<MODEL_BOOZER_VAC, MODE_ADAPTIVE>(n, blocks, threads);
-    case MODEL_BOOZER_SAW: return split_shape<MODEL_BOOZER_SAW, MODE_ADAPTIVE>(n, blocks, threads);
-    default: return split_shape<MODEL_CART, MODE_ADAPTIVE>(n, blocks, threads);
+    case MODEL_BOOZER_VAC: return trace_shape<MODEL_BOOZER_VAC, MODE_ADAPTIVE>(n, blocks, threads);
+    case MODEL_BOOZER_SAW: return trace_shape<MODEL_BOOZER_SAW, MODE_ADAPTIVE>(n, blocks, threads);
+    default: return trace_shape<MODEL_CART, MODE_ADAPTIVE>(n, blocks, threads);
   }
 }
 

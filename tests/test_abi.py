@@ -26,11 +26,27 @@ def test_exports_every_declared_symbol(lib):
     for name in declared:
         assert hasattr(lib, name), name
     assert b"sm_100a" in lib.catapult_version()
+    # the product library exports nothing beyond its header: measurement / test hooks live in the probe library
+    import subprocess
+    syms = subprocess.run(["nm", "-D", "--defined-only", binding.LIB_PATH], capture_output=True, text=True).stdout
+    exported = set(re.findall(r"\b(catapult_[a-z0-9_]+)\b", syms))
+    assert exported == declared, exported ^ declared
+
+
+def test_probe_library_exports_its_header():
+    from paper_2604_07617_b200 import binding
+    hdr = open(os.path.join(ROOT, "include", "catapult_probe.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(catapult_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(binding.PROBE_EXPORTS)
+    P = binding.load_probe()
+    for name in declared:
+        assert hasattr(P, name), name
 
 
 def test_struct_layouts_match_header(lib):
     from paper_2604_07617_b200 import binding
-    assert C.sizeof(binding.FieldDesc) == 4 * 6 + 8 * 6 + 8 * 5
+    assert C.sizeof(binding.FieldDesc) == 4 * (6 + 16) + 8 * 6 + 8 * 5 + 8 * 3
     assert C.sizeof(binding.TraceParams) == 8 * 8 + 8 + 4 * 4 + 8 * 4
 
 
@@ -51,6 +67,13 @@ def test_argument_validation_without_gpu(lib):
         assert lib.catapult_field_build(C.byref(d), dummy, None, C.byref(h)) == binding.EINVAL, b
     d = binding.make_desc(dict(base, I0=1.0))
     assert lib.catapult_field_build(C.byref(d), dummy, None, C.byref(h)) == binding.EUNSUPPORTED
+    # more cells than a 32-bit flat index can carry; column tags: the canonical order or nothing
+    d = binding.make_desc(dict(base, ncell=[2048, 2048, 2048]))
+    assert lib.catapult_field_build(C.byref(d), dummy, None, C.byref(h)) == binding.EINVAL
+    d = binding.make_desc(dict(base, quant=[1, 3, 2, 4]))
+    assert lib.catapult_field_build(C.byref(d), dummy, None, C.byref(h)) == binding.EUNSUPPORTED
+    d = binding.make_desc(dict(base, quant=[1, 2, 3, 4]))
+    assert lib.catapult_field_build(C.byref(d), None, None, C.byref(h)) == binding.EINVAL      # tags fine, nodes NULL
     d = binding.make_desc(base)
     assert lib.catapult_field_build(C.byref(d), None, None, C.byref(h)) == binding.EINVAL
     p = binding.make_params(fd["params"])

@@ -86,7 +86,8 @@ struct TraceTraits {
 constexpr int KIND_START = 6;
 constexpr int REQ_QUIT = 1 << 4;
 // named barriers (0 is __syncthreads')
-constexpr int BAR_A = 1, BAR_D = 2, BAR_G = 3 /* and 4: by round parity */, BAR_D2 = 5, BAR_G2 = 6;
+constexpr int BAR_A = 1, BAR_D = 2, BAR_G = 3 /* and 4: by round parity */, BAR_D2 = 5, BAR_G2 = 6, BAR_P = 7;
+constexpr int NT_P = 32 * 5;  // barrier P: the scalar warp and the four contraction warps that own a state component
 
 __device__ __forceinline__ void bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
@@ -122,16 +123,29 @@ __device__ __forceinline__ void mbar_wait(unsigned mbar, unsigned parity) {
   } while (!done);
 }
 
-// two rows (64 contiguous bytes) of the shared half as one batch of loads
-__device__ __forceinline__ void lds_rows2(unsigned addr, double (&v)[8]) {
+// one row (32 contiguous bytes) of the shared half
+__device__ __forceinline__ void lds_row(unsigned addr, double (&v)[4]) {
   asm volatile(
-      "ld.shared.v2.f64 {%0,%1}, [%8];\n\t"
-      "ld.shared.v2.f64 {%2,%3}, [%8+16];\n\t"
-      "ld.shared.v2.f64 {%4,%5}, [%8+32];\n\t"
-      "ld.shared.v2.f64 {%6,%7}, [%8+48];"
-      : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]), "=d"(v[4]), "=d"(v[5]), "=d"(v[6]), "=d"(v[7])
+      "ld.shared.v2.f64 {%0,%1}, [%4];\n\t"
+      "ld.shared.v2.f64 {%2,%3}, [%4+16];"
+      : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3])
       : "r"(addr)
       : "memory");
+}
+__device__ __forceinline__ void sts_f64x2(unsigned addr, double a, double b) {
+  asm volatile("st.shared.v2.f64 [%0], {%1,%2};" ::"r"(addr), "d"(a), "d"(b) : "memory");
+}
+
+// sum_{j < NJ} a[NJ][j] k_j: the part of stage state NJ + 2 (row NJ of DP_A) that is known before k_NJ is
+template <int NJ>
+__device__ __forceinline__ double stage_partial(const double* ks) {  // ks: this lane's component, stride 128
+  double k[NJ];
+#pragma unroll
+  for (int j = 0; j < NJ; ++j) k[j] = ks[j * 128];  // the loads first, then the sum (j ascending, as everywhere)
+  double p = 0.0;
+#pragma unroll
+  for (int j = 0; j < NJ; ++j) p = fma(DP_A[NJ][j], k[j], p);
+  return p;
 }
 
 // ---- contraction warps -----------------------------------------------------------------------------------------
@@ -146,7 +160,6 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
   const unsigned strip_s = smem_u32(strip);
   const unsigned mbar = smem_u32(smem + TT::OFF_MBAR) + 8u * (q * 32 + lane);
   const double* wbuf = reinterpret_cast<const double*>(smem + TT::OFF_W);
-  double2* part = reinterpret_cast<double2*>(smem + TT::OFF_PART) + (q * 2) * 32 + lane;
   const volatile int* reqbuf = reinterpret_cast<const volatile int*>(smem + TT::OFF_REQ);
   const volatile long long* gbuf = reinterpret_cast<const volatile long long*>(smem + TT::OFF_G);
   const volatile int* g2buf = reinterpret_cast<const volatile int*>(smem + TT::OFF_G2);
@@ -178,14 +191,15 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
     bulk_g2s(strip_s, src + 32, 256, mbar);
     pending = true;
   };
-  // P_a = sum_bc C[a][b][c] wS^b wF^c for a = 0..3 (horner_plane of gc_device.cuh: same operations, same order;
-  // the shared half comes two rows at a time, rows b = 2, 3 of a plane before its rows b = 0, 1)
+  // P_a = sum_bc C[a][b][c] wS^b wF^c for a = 0..3 (horner_plane of gc_device.cuh: same operations, same order).
+  // The shared half streams through two 4-register row buffers, one row in flight while the other is worked
+  // on, rows b = 3, 2, 1, 0 of a plane in turn (Horner in wS); the register half fills the gaps.
+  const unsigned part_s = smem_u32(smem + TT::OFF_PART) + ((q * 2) * 32 + lane) * 16;
   auto contract = [&](double wF, double wS) {
-    double v[8];
-    lds_rows2(strip_s + 64, v);  // plane 2, rows 2, 3
-    double P[2];
-#pragma unroll
-    for (int a = 0; a < 2; ++a) {
+    double va[4], vb[4];
+    lds_row(strip_s + 3 * 32, va);  // plane 2, row 3
+    lds_row(strip_s + 2 * 32, vb);  // plane 2, row 2
+    auto plane_reg = [&](int a) {
       double row[4];
 #pragma unroll
       for (int b = 0; b < 4; ++b) row[b] = reg[(a * 4 + b) * 4 + 3];
@@ -193,28 +207,35 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
       for (int c = 2; c >= 0; --c)
 #pragma unroll
         for (int b = 0; b < 4; ++b) row[b] = fma(row[b], wF, reg[(a * 4 + b) * 4 + c]);
-      P[a] = horner_row(row[0], row[1], row[2], row[3], wS);
-    }
-    part[0] = make_double2(P[0], P[1]);
-#pragma unroll
-    for (int a = 0; a < 2; ++a) {
-      const double r3 = horner_row(v[4], v[5], v[6], v[7], wF);
-      const double r2 = horner_row(v[0], v[1], v[2], v[3], wF);
-      lds_rows2(strip_s + 128 * a, v);  // rows 0, 1 of this plane
-      double acc = fma(r3, wS, r2);
-      const double r1 = horner_row(v[4], v[5], v[6], v[7], wF);
-      const double r0 = horner_row(v[0], v[1], v[2], v[3], wF);
-      if (a == 0) lds_rows2(strip_s + 128 + 64, v);  // plane 3, rows 2, 3
-      acc = fma(acc, wS, r1);
-      P[a] = fma(acc, wS, r0);
-    }
-    part[32] = make_double2(P[0], P[1]);
+      return horner_row(row[0], row[1], row[2], row[3], wS);
+    };
+    const double P0 = plane_reg(0);
+    double acc = horner_row(va[0], va[1], va[2], va[3], wF);
+    lds_row(strip_s + 1 * 32, va);  // plane 2, row 1
+    acc = fma(acc, wS, horner_row(vb[0], vb[1], vb[2], vb[3], wF));
+    lds_row(strip_s + 0 * 32, vb);  // plane 2, row 0
+    const double P1 = plane_reg(1);
+    sts_f64x2(part_s, P0, P1);
+    acc = fma(acc, wS, horner_row(va[0], va[1], va[2], va[3], wF));
+    lds_row(strip_s + 7 * 32, va);  // plane 3, row 3
+    const double P2 = fma(acc, wS, horner_row(vb[0], vb[1], vb[2], vb[3], wF));
+    lds_row(strip_s + 6 * 32, vb);  // plane 3, row 2
+    acc = horner_row(va[0], va[1], va[2], va[3], wF);
+    lds_row(strip_s + 5 * 32, va);  // plane 3, row 1
+    acc = fma(acc, wS, horner_row(vb[0], vb[1], vb[2], vb[3], wF));
+    lds_row(strip_s + 4 * 32, vb);  // plane 3, row 0
+    acc = fma(acc, wS, horner_row(va[0], va[1], va[2], va[3], wF));
+    const double P3 = fma(acc, wS, horner_row(vb[0], vb[1], vb[2], vb[3], wF));
+    sts_f64x2(part_s + 32 * 16, P2, P3);
   };
 
   for (;;) {
     bar_sync(BAR_A, NT);
     const int rq = reqbuf[lane];
-    if (rq & REQ_QUIT) break;  // block-uniform
+    if (rq & REQ_QUIT) {  // block-uniform
+      wait_strip();    // nothing may still be landing in shared memory when the block retires
+      break;
+    }
     const bool active = rq & 1;
     const int kind = (rq >> 1) & 7;  // block-uniform
     const int rpar = (rq >> 6) & 1;
@@ -223,27 +244,35 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
       wait_strip();
       contract(wF, wS);
     }
+    __syncwarp();
+    bar_arrive(BAR_D, NT);
     // ---- stage algebra of state component q: what the next round's stage state needs of the
     // derivatives known so far; in the last round of an attempt everything of Eq. 4 that does not
     // need the last derivative: c = (1,1,1,v_total), state and derivative at the start of the step
     if (q < 4 && kind < KIND_START) {
-      if (kind < 5) {
-        double p = 0.0;
-        for (int j = 0; j <= kind; ++j) p = fma(DP_A[kind + 1][j], ks[j * 128], p);
-        pbuf[0] = p;
-      } else {
-        double e = 0.0;
+      switch (kind) {
+        case 0: pbuf[0] = stage_partial<1>(ks); break;
+        case 1: pbuf[0] = stage_partial<2>(ks); break;
+        case 2: pbuf[0] = stage_partial<3>(ks); break;
+        case 3: pbuf[0] = stage_partial<4>(ks); break;
+        case 4: pbuf[0] = stage_partial<5>(ks); break;
+        default: {
+          double k[6];
 #pragma unroll
-        for (int j = 0; j < 6; ++j)
-          if (j != 1) e = fma(DP_E[j], ks[j * 128], e);
-        errbuf[0] = e;
-        const double sc = (q == 3) ? tc.atol * tc.vtot : tc.atol;
-        const double ah = fabs(ysm[4 * 32]);
-        errbuf[4 * 32] = fm::rcp(fma(tc.rtol, fma(ah, fabs(ks[0]), fabs(ysm[q * 32])), sc));
+          for (int j = 0; j < 6; ++j) k[j] = ks[j * 128];
+          double e = 0.0;
+#pragma unroll
+          for (int j = 0; j < 6; ++j)
+            if (j != 1) e = fma(DP_E[j], k[j], e);
+          errbuf[0] = e;
+          const double sc = (q == 3) ? tc.atol * tc.vtot : tc.atol;
+          const double ah = fabs(ysm[4 * 32]);
+          errbuf[4 * 32] = fm::rcp(fma(tc.rtol, fma(ah, fabs(k[0]), fabs(ysm[q * 32])), sc));
+        }
       }
+      __syncwarp();
+      bar_arrive(BAR_P, NT_P);
     }
-    __syncwarp();
-    bar_arrive(BAR_D, NT);
     // ---- the scalar warp has located the point: a wrong cell is redone; then the guessed cell of the next
     // point is fetched while the scalar warp works on
     bar_sync(BAR_G + rpar, NT);
@@ -674,6 +703,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
         // stage state y + h sum_{j<=r} a[r][j] k_j (row 5 = b: the new state); the sum over j < r was
         // accumulated by the contraction warps during the previous round, the newest derivative enters last
         const double ad = DP_A[r][r];
+        if (r > 0) bar_sync(BAR_P, NT_P);
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           const double Pc = r > 0 ? pbuf[c * 32] : 0.0;
@@ -687,6 +717,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
       rounds += 6;
       // PAPER.md:85 Eq. 4: the contraction warps left the sums over the first six derivatives and the
       // reciprocal denominators
+      bar_sync(BAR_P, NT_P);
       double r = 0.0, chk = 0.0;
 #pragma unroll
       for (int c = 0; c < 4; ++c) {

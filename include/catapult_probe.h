@@ -26,7 +26,9 @@ catapult_status catapult_measure_l2_bandwidth(size_t bytes, double *bytes_per_s)
    exists):
      ATAN2: out0 = atan2(a, b);  SINCOS: out0 = sin(a), out1 = cos(a);  EXP: out0 = exp(a);
      SQRT_RSQRT: out0 = sqrt(a), out1 = 1/sqrt(a);  RCP: out0 = 1/a;
-     POW_NEG_INV: out0 = a^(-1/5), out1 = a^(-1/3) (the step-size controller's powers).
+     POW_NEG_INV: out0 = a^(-1/5), out1 = a^(-1/3) (the step-size controller's powers);
+     CONTROLLER: the tracer's step-size controller itself (S2) for an attempted step of
+       length 1 with error ratio a and maximum step b: out0 = next step length, out1 = 1 if accepted else 0.
    d_b and d_out1 may be NULL where unused. */
 #define CATAPULT_FN_ATAN2 0
 #define CATAPULT_FN_SINCOS 1
@@ -34,6 +36,7 @@ catapult_status catapult_measure_l2_bandwidth(size_t bytes, double *bytes_per_s)
 #define CATAPULT_FN_SQRT_RSQRT 3
 #define CATAPULT_FN_RCP 4
 #define CATAPULT_FN_POW_NEG_INV 5
+#define CATAPULT_FN_CONTROLLER 6
 catapult_status catapult_math_probe(int32_t fn, int64_t n, const double *d_a, const double *d_b,
                                     double *d_out0, double *d_out1, void *stream);
 

@@ -22,6 +22,8 @@
  *       n*H - omega*P_zeta with a wave.
  *   orc_gc_cartesian (R3)        : pure toroidal field closed form; energy;
  *       P_phi in an axisymmetric field.
+ *   orc_default_steps            : hand values of reading S3 (9.37e-7 s for config 0, |G|/|B|(node 0) and R_max
+ *       retyped from the constants), explicit values win, dt0 clamped to dtmax.
  *   orc_trace                    : brute-force fixed-step RK4 on a tiny ensemble.
  *   orc_estimate                 : numpy.mean.
  * Parity unpinned: absolute loss fractions of the five configs (nothing in the

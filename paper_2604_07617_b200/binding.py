@@ -369,7 +369,7 @@ def catapult_estimate(g_kind: int, d_status=None, d_tstop=None, d_g_user=None, t
     return h if to_host else out
 
 
-FN_ATAN2, FN_SINCOS, FN_EXP, FN_SQRT_RSQRT, FN_RCP, FN_POW_NEG_INV = range(6)
+FN_ATAN2, FN_SINCOS, FN_EXP, FN_SQRT_RSQRT, FN_RCP, FN_POW_NEG_INV, FN_CONTROLLER = range(7)
 
 
 def catapult_math_probe(fn: int, d_a, d_b=None):

@@ -1,6 +1,6 @@
 // Test hook: evaluates the device-side elementary functions of gc_math.cuh on arrays, so that
 // tests/test_gpu_parity.py can compare them with numpy on the argument ranges the tracer uses.
-#include "gc_math.cuh"
+#include "gc_device.cuh"
 #include "catapult_probe.h"
 #include "internal.h"
 
@@ -18,6 +18,12 @@ __global__ void math_probe_kernel(int fn, long long n, const double* __restrict_
       case CATAPULT_FN_SQRT_RSQRT: fm::sqrt_rsqrt(x, r0, r1); break;
       case CATAPULT_FN_RCP: r0 = fm::rcp(x); break;
       case CATAPULT_FN_POW_NEG_INV: r0 = fm::pow_neg_inv(x, true); r1 = fm::pow_neg_inv(x, false); break;
+      case CATAPULT_FN_CONTROLLER: {  // the tracer's step-size controller for an attempted step of length 1
+        bool accepted;
+        r0 = controller(1.0, x, y, accepted);
+        r1 = accepted ? 1.0 : 0.0;
+        break;
+      }
       default: break;
     }
     o0[i] = r0;

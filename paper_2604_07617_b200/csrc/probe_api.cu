@@ -34,9 +34,10 @@ const char* catapult_probe_last_error(void) { return g_probe_error.c_str(); }
 catapult_status catapult_math_probe(int32_t fn, int64_t n, const double* d_a, const double* d_b, double* d_out0,
                                     double* d_out1, void* stream) {
   if (n < 0) return fail(CATAPULT_EINVAL, "n < 0");
-  if (fn < 0 || fn > CATAPULT_FN_POW_NEG_INV) return fail(CATAPULT_EINVAL, "unknown fn");
+  if (fn < 0 || fn > CATAPULT_FN_CONTROLLER) return fail(CATAPULT_EINVAL, "unknown fn");
   if (n > 0 && (!d_a || !d_out0)) return fail(CATAPULT_EINVAL, "d_a/d_out0 is NULL");
-  if (n > 0 && fn == CATAPULT_FN_ATAN2 && !d_b) return fail(CATAPULT_EINVAL, "atan2 needs d_b");
+  if (n > 0 && (fn == CATAPULT_FN_ATAN2 || fn == CATAPULT_FN_CONTROLLER) && !d_b)
+    return fail(CATAPULT_EINVAL, "atan2 / controller need d_b");
   return launch_math_probe(fn, n, d_a, d_b, d_out0, d_out1, (cudaStream_t)stream);
 }
 

@@ -128,22 +128,49 @@ def test_field_eval_parity(K, oracle, cases, idx):
 def test_single_step_parity(K, oracle, cases, idx):
     c = cases[idx]
     cfg = c["cfg"]
-    x0 = cfg["x0"]
+    x0 = cfg["x0"].copy()
     n = x0.shape[1]
     rng = np.random.default_rng(200 + idx)
     t = 1e-6 * rng.random(n)
-    h = cfg["params"]["dtmax"] * (0.02 + 0.1 * rng.random(n))
+    # step lengths from 2 % of dtmax up to dtmax itself (the controller's cap)
+    h = cfg["params"]["dtmax"] * np.where(np.arange(n) % 3 == 0, 0.3 + 0.7 * rng.random(n), 0.02 + 0.1 * rng.random(n))
+    h[0] = cfg["params"]["dtmax"]
+    if cfg["field"]["coord"] == 0:
+        # near the magnetic axis: the first s-cell, where the pseudo-Cartesian map is there for
+        x0[0, 1::8] = 1e-3
+        x0[0, 2::8] = 0.02
     xg, rg, kg = K.catapult_step_once(c["gf"], cfg["params"], _dev(x0), _dev(t), _dev(h))
     xg, rg, kg = xg.cpu().numpy(), rg.cpu().numpy(), kg.cpu().numpy()
     sc = _state_scale(cfg["field"]["coord"])
+    worst_r = 0.0
     for i in range(n):
         xo, ro, ko = oracle.step_once(c["of"], c["op"], x0[:, i], t[i], h[i])
-        d = _state_diff(cfg["field"]["coord"], xg[:, i], xo)
-        assert np.all(np.abs(d) <= 1e-11 * sc), (i, d)
+        # compared in the stepped variables: near the axis theta itself is ill-conditioned
+        d = _stepped(cfg["field"]["coord"], xg[:, i]) - _stepped(cfg["field"]["coord"], xo)
         kscale = np.abs(ko).max(axis=0)
-        assert np.all(np.abs(kg[:, :, i] - ko) <= 1e-11 * kscale[None, :] + 1e-300), (i,)
-        # the error ratio is a quotient of a cancellation-prone difference: compare loosely
-        assert abs(rg[i] - ro) <= 1e-3 * max(ro, 1e-3), (i, rg[i], ro)
+        tol_x, tol_k = 1e-11 * sc, 1e-11 * kscale[None, :] + 1e-300
+        if h[i] > 0.2 * cfg["params"]["dtmax"]:
+            # A step of this length is far outside the method's range (error ratio >> 1, stage points leave the
+            # grid and extrapolate): where the extrapolated |B| passes near zero the attempt is
+            # ill-conditioned in any arithmetic.  The bar stays 1e-11 unless the ORACLE's own result moves by more
+            # than that when its input state moves by one unit in the last place.
+            sens_x, sens_k = np.zeros(4), np.zeros_like(ko)
+            for comp in range(4):
+                for direction in (-np.inf, np.inf):
+                    xp = x0[:, i].copy()
+                    xp[comp] = np.nextafter(xp[comp], direction)
+                    xq, _, kq = oracle.step_once(c["of"], c["op"], xp, t[i], h[i])
+                    sens_x = np.maximum(sens_x, np.abs(_stepped(cfg["field"]["coord"], xq) - _stepped(cfg["field"]["coord"], xo)))
+                    sens_k = np.maximum(sens_k, np.abs(kq - ko))
+            tol_x, tol_k = np.maximum(tol_x, 8 * sens_x), np.maximum(tol_k, 8 * sens_k)
+        assert np.all(np.abs(d) <= tol_x), (i, d, tol_x)
+        assert np.all(np.abs(kg[:, :, i] - ko) <= tol_k), (i,)
+        # Eq. 4's error ratio drives the controller: a 1-ulp change of the state moves it by < 1e-5
+        # relative (measured with the oracle), so 1e-4 is what the arithmetic supports
+        rel = abs(rg[i] - ro) / max(ro, 1e-3)
+        worst_r = max(worst_r, rel)
+        assert rel <= 1e-4, (i, rg[i], ro)
+    print(f"cfg{idx}: single step, worst relative difference of the error ratio {worst_r:.2e}")
 
 
 # ---- whole trajectories over the 1e-5 s window ----------------------------------------------------
@@ -175,8 +202,11 @@ def test_trajectory_parity_1e5_window(K, oracle, cases, idx):
     kernel, controller bypassed), so the comparison holds no floating-point decision."""
     c = cases[idx]
     cfg = c["cfg"]
-    x0 = cfg["x0"]
+    x0 = cfg["x0"].copy()
     n = x0.shape[1]
+    if cfg["field"]["coord"] == 0:        # near the magnetic axis too (first s-cell)
+        x0[0, 3::16] = 1e-3
+        x0[0, 4::16] = 0.02
     recs = [oracle.trace_record(c["of"], c["op"], x0[:, i]) for i in range(n)]
     hs = [np.diff(r[0][:, 0]) for r in recs]
     nsteps = max(len(h) for h in hs) + 1          # + 1: every script ends with an h = 0 terminator
@@ -186,7 +216,7 @@ def test_trajectory_parity_1e5_window(K, oracle, cases, idx):
     g = K.catapult_trace_scripted(c["gf"], cfg["params"], _dev(x0), _dev(H))
     gx, gt, gs, gr = (g[k].cpu().numpy() for k in ("xf", "tstop", "status", "r"))
     sc = _state_scale(cfg["field"]["coord"])
-    worst = 0.0
+    worst = worst_r = 0.0
     for i in range(n):
         xo, to, so, ro = oracle.trace_scripted(c["of"], c["op"], x0[:, i], hs[i])
         assert gs[i] == so == recs[i][2]
@@ -195,11 +225,13 @@ def test_trajectory_parity_1e5_window(K, oracle, cases, idx):
         rel = np.abs(d) / np.maximum(sc, np.abs(xo))
         worst = max(worst, rel.max())
         assert np.all(rel <= 1e-8), (i, rel)
-        # the error ratio of every step taken (cancellation-prone: loose) and nothing beyond the script
+        # the error ratio of every step taken (1e-4: see test_single_step_parity) and nothing beyond the script
         k = len(ro)
-        assert np.all(np.abs(gr[:k, i] - ro) <= 5e-2 * np.maximum(ro, 1e-3)), i
+        rel_r = np.abs(gr[:k, i] - ro) / np.maximum(ro, 1e-3)
+        worst_r = max(worst_r, rel_r.max() if k else 0.0)
+        assert np.all(rel_r <= 1e-4), (i, rel_r.max())
         assert np.all(np.isnan(gr[k:, i]))
-    print(f"cfg{idx}: scripted 1e-5 s window, worst relative difference {worst:.2e}")
+    print(f"cfg{idx}: scripted 1e-5 s window, worst relative difference {worst:.2e}, of the error ratio {worst_r:.2e}")
 
 
 @pytest.mark.parametrize("idx", [0, 1, 2, 3, 4])
@@ -225,14 +257,64 @@ def test_adaptive_trace_1e5_window(K, oracle, cases, idx):
         assert qg[comp, alive].max() <= max(1.0, 3.0 * qo[comp, alive].max()), (comp, qg[comp].max(), qo[comp].max())
     assert np.all(gt[alive] == cfg["params"]["T"])
     assert np.allclose(gt[~alive], o["tstop"][~alive], rtol=0.05)
-    # step counts are integers decided by floating point: close, not identical
+    # Step counts are integers decided by floating point (reading Q13).  On the tabulated Boozer fields the step
+    # sequence is chaotic: the oracle ALONE changes the counts of ~90 % of these particles when rtol moves by 1e-12
+    # (tests/test_oracle_trace.py::test_step_sequences_are_not_reproducible_across_arithmetics), so no second
+    # arithmetic can reproduce them; the same perturbation is repeated here and the GPU run must agree with the
+    # oracle at least as often as the oracle agrees with itself (minus three particles).  In config 3's smooth
+    # field the counts ARE reproducible: there >= 90 % of the particles must match the oracle's counts exactly and
+    # its end state to 1e-8.  (Equal counts alone do not mean equal sequences: two different decisions can cancel.)
     na, nr = g["nacc"].cpu().numpy(), g["nrej"].cpu().numpy()
+    same = (na == o["nacc"]) & (nr == o["nrej"])
+    sc = _state_scale(coord)
+    dz = _stepped(coord, gx) - _stepped(coord, o["xf"])
+    rel = np.abs(dz) / np.maximum(sc[:, None], np.abs(_stepped(coord, o["xf"])))
+    close = np.all(rel <= 1e-8, axis=0)
+    o2 = oracle.trace(c["of"], oracle.make_params(dict(cfg["params"], rtol=rtol * (1 + 1e-12))), cfg["x0"])
+    self_same = (o2["nacc"] == o["nacc"]) & (o2["nrej"] == o["nrej"])
+    attempts = int(o["nacc"].sum() + o["nrej"].sum())
+    print(f"cfg{idx}: adaptive run, {np.sum(same)}/{len(same)} particles with the oracle's exact step counts "
+          f"({attempts} attempts; the oracle against itself at rtol (1 + 1e-12): {np.sum(self_same)}/{len(same)}); worst "
+          f"relative end-state difference where the counts match {rel[:, same].max() if same.any() else 0.0:.2e}")
+    assert np.sum(same) >= np.sum(self_same) - 3, (np.sum(same), np.sum(self_same))
+    if coord == 1:
+        assert np.mean(same & close) >= 0.9, np.mean(same & close)
     assert abs(na.sum() / o["nacc"].sum() - 1) < 0.02 and abs((nr.sum() + 1) / (o["nrej"].sum() + 1) - 1) < 0.1
     assert np.abs(na.astype(int) - o["nacc"].astype(int)).max() <= 0.1 * o["nacc"].max() + 3
     cnt = g["counters"].cpu().numpy()
     assert cnt[0] == na.sum() and cnt[1] == nr.sum()
     assert cnt[2] == np.sum(gs == 0) and cnt[3] == np.sum(gs == 1)
     assert cnt[6] >= 6 * (na.sum() + nr.sum())
+
+
+@pytest.mark.parametrize("idx", [0, 2, 3])
+def test_default_step_lengths_resolved_on_the_device(K, oracle, cases, idx):
+    """dt0 = dtmax = 0 selects reading S3's defaults.  For a Boozer grid they need |B|(node 0), which the field
+    build leaves on the device; the tracer resolves them itself.  catapult_trace_init hands back the initial step
+    it resolved: bit-exact against orc_default_steps (pinned by hand values); the whole trace then matches the
+    oracle's run with the same defaults."""
+    c = cases[idx]
+    cfg = c["cfg"]
+    pd = dict(cfg["params"], dt0=0.0, dtmax=0.0)
+    dt0_o, dtmax_o = oracle.default_steps(c["of"], oracle.make_params(pd))
+    st = K.catapult_trace_init(c["gf"], pd, _dev(cfg["x0"]).clone())
+    assert torch.all(st["dt"] == dt0_o), (st["dt"][0].item(), dt0_o)
+    # an explicit dt0 above the default dtmax is clamped to it: exposes the device-side dtmax bit-exactly too
+    st2 = K.catapult_trace_init(c["gf"], dict(pd, dt0=1.0), _dev(cfg["x0"]).clone())
+    assert torch.all(st2["dt"] == dtmax_o), (st2["dt"][0].item(), dtmax_o)
+    g = K.catapult_trace(c["gf"], pd, _dev(cfg["x0"]))
+    o = oracle.trace(c["of"], oracle.make_params(pd), cfg["x0"])
+    assert np.array_equal(g["status"].cpu().numpy(), o["status"])
+    na, nr = g["nacc"].cpu().numpy(), g["nrej"].cpu().numpy()
+    if cfg["field"]["coord"] == 1:      # reproducible step sequences only in the smooth field (reading Q13)
+        assert np.mean((na == o["nacc"]) & (nr == o["nrej"])) >= 0.9
+    assert abs(na.sum() / o["nacc"].sum() - 1) < 0.02
+    ref = oracle.trace(c["of"], oracle.make_params(dict(pd, rtol=1e-12, atol=1e-15)), cfg["x0"])
+    coord = cfg["field"]["coord"]
+    q = _free_diff_over_tol(coord, g["xf"].cpu().numpy(), ref["xf"], o["nacc"].astype(float), pd["rtol"])
+    qo = _free_diff_over_tol(coord, o["xf"], ref["xf"], o["nacc"].astype(float), pd["rtol"])
+    alive = o["status"] == 0
+    assert q[:, alive].max() <= max(1.0, 3.0 * qo[:, alive].max())
 
 
 def test_cfg0_full_statistics(K, oracle):
@@ -505,6 +587,38 @@ def test_estimate_parity(K, oracle):
             assert np.allclose(got, want, rtol=1e-12, atol=1e-300)
     with pytest.raises(K.CatapultError):
         K.catapult_estimate(0, d_status=None, d_tstop=_dev(np.zeros(3)))
+
+
+def test_controller_parity(K, oracle):
+    """The tracer's step-size controller ("matching the implementation in Boost"; S2) against
+    orc_controller (pinned by a hand table in tests/test_oracle_dp5.py) on the thresholds, the floors and the cap:
+    the accept / reject decision exactly, the next step length to 1e-14."""
+    r = np.array([0.0, 1e-300, 1e-12, 1e-6, 3.1e-4, 3.2e-4, 3.3e-4, 0.1, 0.4, 0.5 - 1e-16, 0.5, 0.5 + 1e-16, 0.75,
+                  1.0 - 1e-16, 1.0, 1.0 + 3e-16, 1.5, 8.0, 91.125, 91.2, 1e3, 1e6, 1e30, np.inf, np.nan])
+    rng = np.random.default_rng(5)
+    r = np.concatenate([r, 10.0 ** rng.uniform(-8, 4, 4000)])
+    for cap in (1e300, 4.5, 3.0, 1.0, 0.25):
+        dtn, acc = (t.cpu().numpy() for t in K.catapult_math_probe(K.FN_CONTROLLER, _dev(r), _dev(np.full(r.shape, cap))))
+        want = np.array([oracle.controller(1.0, float(v), cap) for v in r])
+        assert np.array_equal(acc, want[:, 1]), np.flatnonzero(acc != want[:, 1])
+        assert np.all(np.abs(dtn - want[:, 0]) <= 1e-14 * want[:, 0]), np.abs(dtn / want[:, 0] - 1).max()
+
+
+@pytest.mark.parametrize("idx", [0, 2, 3, 4])
+def test_first_attempts_follow_the_oracle_exactly(K, oracle, cases, idx):
+    """Before the step sequence has had time to diverge (reading Q13) the adaptive kernel must walk the oracle's own
+    sequence: after N = 1..8 attempts every particle has the oracle's accepted / rejected counts, and the
+    time reached agrees to 2e-5 (the step length inherits the error ratio's sensitivity, ~1e-5)."""
+    c = cases[idx]
+    cfg = c["cfg"]
+    for N in (1, 2, 3, 5, 8):
+        pd = dict(cfg["params"], max_steps=N)
+        st = K.catapult_trace_init(c["gf"], pd, _dev(cfg["x0"]).clone())
+        K.catapult_trace_continue(c["gf"], pd, st)
+        o = oracle.trace(c["of"], oracle.make_params(pd), cfg["x0"])
+        assert np.array_equal(st["nacc"].cpu().numpy(), o["nacc"]) and np.array_equal(st["nrej"].cpu().numpy(), o["nrej"]), N
+        assert np.array_equal(st["status"].cpu().numpy(), o["status"])
+        assert np.allclose(st["t"].cpu().numpy(), o["tstop"], rtol=2e-5, atol=0.0), N
 
 
 def test_device_math_parity(K):

@@ -182,3 +182,75 @@ def test_scripted_replay_reproduces_the_adaptive_trace(oracle):
             if idx != 3:
                 de[1] = math.remainder(de[1], 2 * math.pi)   # theta is returned in (-pi, pi]
             assert te == 0.0 and len(re) == 0 and np.all(np.abs(de) <= 1e-15 * np.maximum(1.0, np.abs(x0)))
+
+
+def test_default_steps_hand_values(oracle):
+    """Pin of reading S3 (the paper is silent on the initial / maximum step): dtmax = (pi/2) L / v_total,
+    dt0 = 1e-3 dtmax, L = |G| / |B|(first node) for a Boozer grid, L = R_max for the cylindrical grid.
+    Hand values: 3.5 MeV alphas, v_total = 1.29963e7 m/s; config 0 has |B|(node 0) = B0 exactly,
+    so L = R0 = 7.75 m and dtmax = (pi/2) 7.75 / 1.29963e7 = 9.37e-7 s."""
+    O = oracle
+    v = math.sqrt(2.0 * 3.5e6 * 1.602176634e-19 / 6.64e-27)          # retyped from the constants, not from W
+    assert abs(v - 1.29963e7) < 5e2
+    cfg = W.config(0, n=1)
+    p0 = O.make_params(dict(cfg["params"], dt0=0.0, dtmax=0.0))
+    dt0, dtmax = O.default_steps(O.Field(cfg["field"]), p0)
+    assert abs(dtmax - 9.37e-7) < 5e-10                               # the survey's printed three digits
+    assert abs(dtmax / (0.5 * math.pi * 7.75 / v) - 1) < 1e-14 and abs(dt0 / (1e-3 * dtmax) - 1) < 1e-15
+    # a field whose first node is not B0: L follows the node (m = 0 modes shift |B| on the axis)
+    cfg2 = W.config(2, n=1, ncell=[4, 4, 4])
+    b00 = float(cfg2["field"]["nodes"][0, 0, 0, 0])
+    assert abs(b00 / W.B0 - 1) > 1e-3                                 # the case really differs from config 0
+    dt0, dtmax = O.default_steps(O.Field(cfg2["field"]), O.make_params(dict(cfg2["params"], dt0=0.0, dtmax=0.0)))
+    assert abs(dtmax / (0.5 * math.pi * (W.B0 * W.R0 / abs(b00)) / v) - 1) < 1e-14
+    # cylindrical grid: L = R_max = R0 + 1.25 a (reading Q12)
+    cfg3 = W.config(3, n=1, ncell=[4, 4, 2])
+    dt0, dtmax = O.default_steps(O.Field(cfg3["field"]), O.make_params(dict(cfg3["params"], dt0=0.0, dtmax=0.0)))
+    assert abs(dtmax / (0.5 * math.pi * (7.75 + 1.25 * 1.7) / v) - 1) < 1e-14
+    # explicit values win; an explicit dt0 above dtmax is clamped
+    f0 = O.Field(cfg["field"])
+    assert O.default_steps(f0, O.make_params(dict(cfg["params"], dt0=2e-9, dtmax=3e-7))) == (2e-9, 3e-7)
+    assert O.default_steps(f0, O.make_params(dict(cfg["params"], dt0=1e-3, dtmax=3e-7))) == (3e-7, 3e-7)
+    assert O.default_steps(f0, O.make_params(dict(cfg["params"], dt0=5e-9, dtmax=0.0)))[0] == 5e-9
+
+
+def test_default_steps_drive_the_trace(oracle):
+    """orc_trace with dt0 = dtmax = 0 equals orc_trace with the values orc_default_steps returns, bit for bit."""
+    O = oracle
+    cfg = W.config(2, n=6, T=2e-6, ncell=[6, 5, 4])
+    f = O.Field(cfg["field"])
+    pdef = dict(cfg["params"], dt0=0.0, dtmax=0.0)
+    dt0, dtmax = O.default_steps(f, O.make_params(pdef))
+    a = O.trace(f, O.make_params(pdef), cfg["x0"])
+    b = O.trace(f, O.make_params(dict(cfg["params"], dt0=dt0, dtmax=dtmax)), cfg["x0"])
+    assert np.array_equal(a["xf"], b["xf"]) and np.array_equal(a["nacc"], b["nacc"])
+    c = O.trace(f, O.make_params(cfg["params"]), cfg["x0"])          # L = R0 instead of |G|/|B|(node 0): another run
+    assert not np.array_equal(a["nacc"] + a["nrej"], c["nacc"] + c["nrej"]) or not np.array_equal(a["xf"], c["xf"])
+
+
+def test_step_sequences_are_not_reproducible_across_arithmetics(oracle):
+    """Reading Q13, measured with the oracle alone: on the tabulated Boozer fields the sequence of
+    accepted / rejected attempts is chaotic -- the tricubic interpolant's derivative jumps at cell faces make
+    Eq. 4's error ratio a rough function of the step length -- so a relative change of 1e-12 in rtol (less than
+    any two correct arithmetics differ by) changes the step counts of most particles within a 1e-5 s window,
+    while the end states still agree within the method's global error.  In the smooth axisymmetric field of
+    config 3 the counts are reproducible.  This is why the GPU parity of whole trajectories is taken on a scripted
+    step sequence, and the adaptive run is compared per particle only on config 3."""
+    O = oracle
+    out = {}
+    for idx, kw in ((0, dict(n=64, T=1e-5)), (3, dict(n=50, T=1e-5, ncell=[12, 11, 5]))):
+        cfg = W.config(idx, **kw)
+        f = O.Field(cfg["field"])
+        a = O.trace(f, O.make_params(cfg["params"]), cfg["x0"])
+        b = O.trace(f, O.make_params(dict(cfg["params"], rtol=cfg["params"]["rtol"] * (1 + 1e-12))), cfg["x0"])
+        same = (a["nacc"] == b["nacc"]) & (a["nrej"] == b["nrej"])
+        out[idx] = same.mean()
+        # both runs are correct: end states within the global error nacc * rtol of each other
+        ya = np.array([a["xf"][0] * np.cos(a["xf"][1]), a["xf"][0] * np.sin(a["xf"][1]), a["xf"][2], a["xf"][3]]) \
+            if idx == 0 else a["xf"]
+        yb = np.array([b["xf"][0] * np.cos(b["xf"][1]), b["xf"][0] * np.sin(b["xf"][1]), b["xf"][2], b["xf"][3]]) \
+            if idx == 0 else b["xf"]
+        scale = np.maximum(np.array([1.0, 1.0, 1.0, W.V_TOTAL])[:, None], np.abs(ya))
+        assert np.all(np.abs(ya - yb) <= 8 * a["nacc"][None, :] * 1e-9 * scale)
+    assert out[0] < 0.5, out      # measured: 5 of 64 particles keep their counts
+    assert out[3] == 1.0, out     # measured: 50 of 50

@@ -348,33 +348,75 @@ def test_cfg0_full_statistics(K, oracle):
     assert abs(na.sum() / o["nacc"].sum() - 1) < 0.01
 
 
-def test_cfg1_loss_fraction_within_3_sigma(K):
-    """Config 1 at full size (10,000 alphas, T = 1e-3 s, launch shape of bench.py) against the oracle's
-    stored result (tests/golden/cfg1_oracle.txt, written by tests/golden/make_golden.py from oracle/)."""
-    path = os.path.join(GOLDEN, "cfg1_oracle.txt")
+def _golden(idx):
+    path = os.path.join(GOLDEN, f"cfg{idx}_oracle.txt")
     if not os.path.exists(path):
-        pytest.fail("tests/golden/cfg1_oracle.txt missing: run python tests/golden/make_golden.py")
+        pytest.fail(f"tests/golden/cfg{idx}_oracle.txt missing: run python tests/golden/make_golden.py")
     gold = {}
     for line in open(path):
         if line.startswith("#") or not line.strip():
             continue
         k, v = line.split("=", 1)
         gold[k.strip()] = v.strip()
-    n = int(gold["n"])
+    return gold
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 4])
+def test_loss_fraction_within_3_sigma_of_the_oracle(K, oracle, idx):
+    """north_star: "loss fraction within 3 binomial standard deviations at n >= 1e4" on every config with losses.
+    The first 10,000 particles of configs 1-4 on their FULL grids, traced to the T stored with the oracle's result
+    (tests/golden/cfg{idx}_oracle.txt, written by tests/golden/make_golden.py from oracle/ alone; T = 1e-3 s:
+    config 1's own T, and what the CPU oracle affords for configs 2-4).  Beyond ~1e-5 s orbits are chaotic
+    (reading Q13), so the comparison is statistical: loss fraction (the paper's own cross-code
+    check), per-particle loss flags, loss-time distribution (reading S5), accepted-step total."""
+    gold = _golden(idx)
+    n, T = int(gold["n"]), float(gold["T"])
     lost_o = np.array([int(ch) for ch in gold["lost_bits"]], dtype=np.int32)
-    cfg = W.config(1)
-    assert n == cfg["x0"].shape[1] == 10_000
+    cfg = W.config(idx, n=n, T=T)
+    assert cfg["x0"].shape[1] == n == 10_000
     gf = K.catapult_field_build(cfg["field"])
     g = K.catapult_trace(gf, cfg["params"], _dev(cfg["x0"]))
     est = K.catapult_estimate(0, d_status=g["status"])
+    gs, gt = g["status"].cpu().numpy(), g["tstop"].cpu().numpy()
+    assert np.all((gs == 0) | (gs == 1)) and est[2] == np.sum(gs == 1)
     p_o = lost_o.mean()
-    sigma = math.sqrt(p_o * (1 - p_o) / n)
+    sigma = math.sqrt(max(p_o * (1 - p_o), 1.0 / n) / n)
+    print(f"cfg{idx}: loss fraction GPU {est[0]:.4f} oracle {p_o:.4f} (sigma {sigma:.4f}); per-particle agreement "
+          f"{np.mean((gs == 1) == (lost_o == 1)):.4f}; accepted steps GPU/oracle "
+          f"{g['nacc'].sum().item() / float(gold['nacc_sum']):.5f}")
     assert abs(est[0] - p_o) <= 3 * sigma, (est[0], p_o, sigma)
-    gs = g["status"].cpu().numpy()
-    assert est[2] == np.sum(gs == 1)
     # per-particle agreement is far better than binomial noise: most orbits are not near the edge
-    assert np.mean((gs == 1) == (lost_o == 1)) > 0.97
+    assert np.mean((gs == 1) == (lost_o == 1)) >= 0.97
     assert abs(g["nacc"].sum().item() / float(gold["nacc_sum"]) - 1) < 0.01
+    assert np.all(gt[gs == 0] == T)
+    if p_o > 0:
+        # loss times: tau is the end of the first accepted step beyond the boundary (reading S5); the distribution of
+        # the ~4000 loss times must agree (quartiles within 10 %: the two lost sets differ by a few per cent of
+        # chaotic orbits), the earliest quartile, lost before chaos sets in, much closer
+        qo = np.array([float(v) for v in gold["tstop_lost_quartiles"].split()])
+        qg = np.quantile(gt[gs == 1], [0.25, 0.5, 0.75])
+        assert np.all(np.abs(qg / qo - 1) < 0.10), (qg, qo)
+        assert abs(qg[0] / qo[0] - 1) < 0.03, (qg[0], qo[0])
+    else:
+        # config 3: nothing is lost, and the invariants hold on every orbit (energy exactly invariant for any B,
+        # P_phi in an axisymmetric field with R B_phi constant: SURVEY.md 8(c) pins)
+        of = oracle.Field(cfg["field"])
+        x0, xf = cfg["x0"], g["xf"].cpu().numpy()
+
+        def inv(x):
+            R = np.hypot(x[0], x[1])
+            v = oracle.tricubic_many(of, np.array([R, x[2], np.arctan2(x[1], x[0])]))
+            return R, v, np.sqrt(v[0] ** 2 + v[1] ** 2 + v[2] ** 2)
+
+        R0_, v0, B0_ = inv(x0)
+        R1_, v1, B1_ = inv(xf)
+        mu = (W.V_TOTAL ** 2 - x0[3] ** 2) / (2 * B0_)
+        E1 = 0.5 * xf[3] ** 2 + mu * B1_
+        assert np.max(np.abs(E1 / (0.5 * W.V_TOTAL ** 2) - 1)) < 1e-6
+        P0 = W.ALPHA_MASS * R0_ * v0[1] / B0_ * x0[3] + W.ALPHA_CHARGE * v0[6]
+        P1 = W.ALPHA_MASS * R1_ * v1[1] / B1_ * xf[3] + W.ALPHA_CHARGE * v1[6]
+        assert np.max(np.abs(P1 - P0)) < 1e-6 * W.ALPHA_CHARGE * W.PSI_EDGE_CYL
+    gf.destroy()
 
 
 # ---- invariants on the GPU result ------------------------------------------------------------------

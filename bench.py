@@ -2,16 +2,27 @@
 """bench.py -- throughput of the CATAPULT hot path on B200 (contract: see the task statement).
 
     python bench.py --gpus 1 --steps K --warmup W                 # this library (CUDA, C-ABI)
+    python bench.py --gpus N ...                                  # spawns N ranks itself (one per GPU)
+    torchrun --nproc-per-node N ... bench.py --gpus N ...         # or under torchrun
     python bench.py --impl reference --steps K --warmup W         # the CPU oracle, timed as it stands
-    torchrun --nproc-per-node N ... bench.py --gpus N ...         # N ranks, one ensemble per rank (weak)
 
-Workload (default cfg4 = BASELINE.json configs[4], the 10^6-particle config north_star's roofline
-target is quoted on): 64^3-cell random-Fourier Boozer field + shear Alfven wave, 10^6 alphas.
-One "step" = one pass of the whole hot path over one batch: field build (a1) -> DP5 tracing of the
-WHOLE ensemble across one time window of `--window` seconds (a2-a9) -> loss-fraction estimate (a10).
-Consecutive steps trace consecutive windows [j*w, (j+1)*w] of the same job with the state carried on
-the device (catapult_trace_continue), so K steps are K*w seconds of the T = 1e-2 s trace; the full
-job is `--window 1e-2 --steps 1`.  The metric (accepted DP5 steps per second) is intensive.
+Workload (default cfg4 = BASELINE.json configs[4], the 10^6-particle config north_star's roofline target is quoted
+on): 64^3-cell random-Fourier Boozer field + shear Alfven wave, 10^6 alphas per GPU.
+
+WINDOW LEG (the timed K steps; `value`).  One "step" = one pass of the whole hot path over one batch: field build
+(a1) -> DP5 tracing of the WHOLE ensemble across one time window of `--window` seconds (a2-a9) -> loss-fraction
+estimate (a10).  Consecutive steps trace consecutive windows [j*w, (j+1)*w] of the same job with the state carried
+on the device (catapult_trace_continue).  The metric (accepted DP5 steps per second) is intensive.
+
+JOB LEG (`full_job`, the second half of BASELINE.json's metric: particles-to-T per second).  The first
+`--job-particles` particles of the same ensemble traced from t = 0 to the config's own T (1e-2 s) in ONE
+catapult_trace launch: the population thins as particles are lost and the tail runs under-filled, so the job-level
+rate is what a user sees.  `--job-particles -1` traces the full ensemble (cfg4: ~10 GPU-minutes; the lines of those
+runs are committed under profiles/).
+
+N > 1: ONE seeded ensemble of N x particles, split over the ranks by interleaved index, tables
+replicated, no data-path collective; one 24-byte all-reduce of (sum g, sum g^2, n) gives the estimate.  Per-GPU work
+is fixed as N grows ("scaling": "weak").
 """
 from __future__ import annotations
 
@@ -19,11 +30,11 @@ import argparse
 import json
 import math
 import os
+import socket
 import statistics
 import subprocess
 import sys
 import tempfile
-import threading
 import time
 
 import numpy as np
@@ -32,17 +43,25 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+from paper_2604_07617_b200 import sharding as S  # noqa: E402
 from paper_2604_07617_b200 import workloads as W  # noqa: E402
 
 METRIC = "fp64 accepted DP5 steps/sec"
 UNIT = "accepted steps/s"
 
-# Algorithmic FP64 work per right-hand-side evaluation: FMA = 2,
-# add/mul = 1, division/sqrt/atan2/sincos/exp = 1 each.  Tricubic contraction 84 FMA per quantity.
-FLOPS_PER_EVAL = {"boozer_vac": 4 * 168 + 39 + 30 + 46, "boozer_saw": 4 * 168 + 39 + 30 + 110,
-                  "cart": 7 * 168 + 39 + 24 + 75}
-FLOPS_STAGE_ALGEBRA_PER_ATTEMPT = 2 * 4 * (1 + 2 + 3 + 4 + 5 + 5) + 2 * 4 * 6 + 4 * 6 + 12
-BYTES_PER_EVAL = {"boozer_vac": 4 * 512, "boozer_saw": 4 * 512, "cart": 7 * 512}
+# ---- the flop model, in ONE place (DESIGN.md section 7.1 quotes these numbers) ----------------------------------
+# ALGORITHMIC work: per right-hand-side evaluation the tricubic contraction of m quantities at
+# 84 FMA each (FMA = 2 flops), ~30 flops of Lagrange basis, and locate + right-hand side (sqrt / atan2 / sincos /
+# exp / division = 1 flop each): ~100 (Boozer vacuum), ~150 (Boozer + wave), ~120 (Cartesian); per attempted step
+# ~150 flops of stage / error algebra.  `roofline.achieved` and `roofline.frac` use these.
+ALG_FLOPS_PER_EVAL = {"boozer_vac": 4 * 168 + 30 + 100, "boozer_saw": 4 * 168 + 30 + 150, "cart": 7 * 168 + 30 + 120}
+ALG_FLOPS_PER_ATTEMPT = 150
+# EXECUTED work of trace_kernel (its own arithmetic: 63-FMA Horner per quantity in the monomial basis, no Lagrange
+# basis; the scalar warp's and the stage sums' DFMA / DMUL / DADD per evaluation from the ncu instruction mix of the
+# committed capture, profiles/r2_ncu_trace_v6c.md).  `roofline.executed` uses these; stage algebra included.
+EXEC_FLOPS_PER_EVAL = {"boozer_vac": 4 * 126 + 215, "boozer_saw": 4 * 126 + 307, "cart": 7 * 126 + 260}
+BYTES_PER_CELL_VISIT = {"boozer_vac": 4 * 512, "boozer_saw": 4 * 512, "cart": 7 * 512}
+KERNELS_PER_STEP = {"catapult_field_build": 1, "catapult_trace_continue": 1, "catapult_trace": 1, "catapult_estimate": 2}
 
 
 def model_of(cfg) -> str:
@@ -123,20 +142,6 @@ def oracle_sample(cfg, window: float, nsample: int, nthreads: int = 0) -> dict:
                 sample=f"first {x0.shape[1]} particles of {cfg['name']} over [0, {window:g}] s")
 
 
-def reduce_over_ranks(time_value: float, counts, world: int, device):
-    """Whole-job figures of a weak-scaling run: the time is the MAX over ranks, every count the SUM over ranks
-    (each rank traces its own ensemble; there is no data-path collective, only this).  Returns (time, [counts])."""
-    if world <= 1:
-        return float(time_value), [float(c) for c in counts]
-    import torch
-    import torch.distributed as dist
-    t = torch.tensor([float(time_value)], dtype=torch.float64, device=device)
-    c = torch.tensor([float(v) for v in counts], dtype=torch.float64, device=device)
-    dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    dist.all_reduce(c, op=dist.ReduceOp.SUM)
-    return float(t.item()), [float(v) for v in c.tolist()]
-
-
 def run_reference(args, cfg_idx: int):
     """--impl reference: the oracle on the host cores (rank 0 only under torchrun)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -164,7 +169,45 @@ def run_reference(args, cfg_idx: int):
     print(json.dumps(line), flush=True)
 
 
-# ------------------------------------------------------------------------------------------------
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` without torchrun: starts N rank processes (one per GPU) with the torchrun
+    environment (RANK, LOCAL_RANK, WORLD_SIZE, MASTER_ADDR = 127.0.0.1, MASTER_PORT) and waits for them."""
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    procs = []
+    for r in range(args.gpus):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(args.gpus), MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port), NCCL_DEBUG=os.environ.get("NCCL_DEBUG", "WARN"))
+        procs.append(subprocess.Popen([sys.executable, os.path.abspath(__file__), *sys.argv[1:]], env=env))
+    rc = 0
+    for p in procs:
+        rc = rc or p.wait()
+    return rc
+
+
+def committed_capture(model: str) -> dict:
+    """Per-evaluation DRAM / L2 bytes of trace_kernel from the committed `ncu --set full` capture of this kernel
+    (profiles/r2_traffic_v6c.csv; the command is in the .md beside it).  bench.py does not run ncu: the traffic
+    it reports is that capture's per-evaluation figure times the evaluations of its own timed launches."""
+    out = {}
+    try:
+        for line in open(os.path.join(ROOT, "profiles", "r2_traffic_v6c.csv")):
+            f = line.strip().split(",")
+            if len(f) >= 3 and f[0] == model:
+                out[f[1]] = float(f[2])
+    except Exception:
+        pass
+    return out
+
+
+def measured_peaks() -> dict:
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return {}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -173,18 +216,32 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4", choices=W.CONFIG_NAMES)
     ap.add_argument("--window", type=float, default=1e-5, help="seconds of physical time traced per step")
-    ap.add_argument("--particles", type=int, default=0, help="override the particle count (0 = full size)")
-    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--particles", type=int, default=0, help="particles per GPU (0 = the config's full size)")
+    ap.add_argument("--cells", type=int, default=0, help="cells per dimension of the same field (0 = the config's grid): "
+                    "the grid-resolution axis of the paper's sweeps (PAPER.md:100-102)")
+    ap.add_argument("--rtol", type=float, default=0.0, help="tracing tolerance (0 = the config's 1e-9): PAPER.md:100-102")
+    ap.add_argument("--e2e-steps", type=int, default=-1, help="steps of the host-buffer leg (-1 = --steps, 0 = skip)")
+    ap.add_argument("--job-particles", type=int, default=65536,
+                    help="particles of the full-T job leg (0 = skip, -1 = the whole ensemble)")
+    ap.add_argument("--job-T", type=float, default=0.0, help="end time of the job leg (0 = the config's own T)")
     ap.add_argument("--cpu-particles", type=int, default=2048, help="oracle sample for cpu_baseline (0 = skip)")
     ap.add_argument("--ref-particles", type=int, default=1024)
     ap.add_argument("--no-peaks", action="store_true")
-    ap.add_argument("--ncell", type=int, default=0,
-                    help="cells per dimension instead of the workload's grid (0 = the workload's): a coarser grid "
-                         "changes cells less often, which separates the cost of cell fetches from the rest")
+    ap.add_argument("--dry-run-ranks", action="store_true", help="every rank prints its environment and exits")
     args = ap.parse_args()
     cfg_idx = W.CONFIG_NAMES.index(args.workload)
     if args.impl == "reference":
         run_reference(args, cfg_idx)
+        return
+    if args.gpus > 1 and "RANK" not in os.environ:
+        sys.exit(spawn_ranks(args))
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.dry_run_ranks:
+        print(json.dumps({"rank": rank, "local_rank": local, "world_size": world,
+                          "master_addr": os.environ.get("MASTER_ADDR", "127.0.0.1"),
+                          "master_port": os.environ.get("MASTER_PORT")}), flush=True)
         return
 
     import torch
@@ -192,27 +249,31 @@ def main():
 
     from paper_2604_07617_b200 import binding as K
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     K.load()
+    launches = {"n": 0}
+
+    def count(name):
+        launches["n"] += KERNELS_PER_STEP[name]
 
     # ---- inputs: seeded, synthetic, resident in HBM before the timed region ---------------------
-    n = args.particles if args.particles > 0 else None
-    ncell = [args.ncell] * 3 if args.ncell > 0 else None
-    cfg = W.config(cfg_idx, n=n, ncell=ncell, ensemble=rank)     # every rank traces its own ensemble (weak scaling)
+    per_gpu = args.particles if args.particles > 0 else W.FULL_N[cfg_idx]
+    ncell = [args.cells] * 3 if args.cells > 0 else None
+    cfg = W.config(cfg_idx, n=per_gpu * world, ncell=ncell)          # ONE ensemble of world x per_gpu particles
+    if args.rtol > 0:
+        cfg["params"]["rtol"] = args.rtol
     fd, pd = cfg["field"], cfg["params"]
     model = model_of(cfg)
-    npart = cfg["x0"].shape[1]
+    x0 = S.shard_columns(cfg["x0"], rank, world)                     # this rank's share: rank, rank + world, ...
+    npart = x0.shape[1]
     d_nodes = torch.from_numpy(fd["nodes"]).cuda()
-    d_x = torch.from_numpy(cfg["x0"]).cuda()
+    d_x = torch.from_numpy(x0).cuda()
     field = K.catapult_field_build(fd, d_nodes)
-    state = K.catapult_trace_init(field, pd, d_x)
+    state = K.catapult_trace_init(field, pd, d_x.clone())
     torch.cuda.synchronize()
     table_bytes = field.table_bytes
     blocks, threads = K.catapult_trace_launch_shape(field, pd)
@@ -224,6 +285,7 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    # ---- window leg -----------------------------------------------------------------------------
     trace_events = []
 
     def one_step(j: int, timed: bool):
@@ -236,6 +298,7 @@ def main():
         if timed:
             e1.record()
             trace_events.append((e0, e1))
+            count("catapult_field_build"), count("catapult_trace_continue"), count("catapult_estimate")
         est = K.catapult_estimate(0, d_status=state["status"], to_host=False)   # a10
         return f, est
 
@@ -266,14 +329,15 @@ def main():
     for f in fields:
         f.destroy()
     cnt = (state["counters"] - cnt0).cpu().numpy().astype(np.float64)
-    ms_all, (acc_all, att_all, evals_all) = reduce_over_ranks(ms, [cnt[0], cnt[0] + cnt[1], cnt[6]], world, "cuda")
+    ms_all, red = S.reduce_timing(ms, [cnt[0], cnt[0] + cnt[1], cnt[6], cnt[7], cnt[8], cnt[9]], device="cuda")
+    acc_all, att_all, evals_all, loads_all, blocking_all, rounds_all = red
     value = acc_all / (ms_all * 1e-3)
-    loss_fraction = float(est[0].item())
+    e = est.cpu().numpy()
+    loss_fraction, loss_se, n_lost, _, n_all = S.reduce_estimate(e[2], e[3], npart, device="cuda")   # the 24-byte reduce
     alive = int((state["status"] == 0).sum().item())
 
     # ---- roofline of the dominant kernel (trace_kernel), measured live with CUDA events ------------
     trace_s = sum(trace_ms) * 1e-3
-    flops = cnt[6] * FLOPS_PER_EVAL[model] + (cnt[0] + cnt[1]) * FLOPS_STAGE_ALGEBRA_PER_ATTEMPT
     roof = None
     if rank == 0:
         peak_fp64 = l2_bw = None
@@ -281,39 +345,49 @@ def main():
             peak_fp64 = K.catapult_measure_fp64_peak()
             l2_bw = K.catapult_measure_l2_bandwidth(48 << 20)
         nominal = 148 * 64 * 2 * 1.965e9          # 64 DFMA/clk/SM at clocks.max.sm (B200_PROFILING.md)
-        achieved = flops / trace_s / 1e12
         peak = (peak_fp64 or nominal) / 1e12
-        alg_bytes = cnt[6] * BYTES_PER_EVAL[model]
-        roof = {"bound": "alu", "kernel": "trace_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak,
-                "peak_source": "measured DFMA micro-benchmark (catapult_measure_fp64_peak)" if peak_fp64 else
+        alg = (cnt[6] * ALG_FLOPS_PER_EVAL[model] + (cnt[0] + cnt[1]) * ALG_FLOPS_PER_ATTEMPT) / trace_s / 1e12
+        exe = cnt[6] * EXEC_FLOPS_PER_EVAL[model] / trace_s / 1e12
+        cap = committed_capture(model)
+        evals_per_launch = cnt[6] / max(1, args.steps)
+        dram_b, l2_b = cap.get("dram_bytes_per_rhs_eval"), cap.get("l2_bytes_per_rhs_eval")
+        roof = {"bound": "alu", "kernel": "trace_kernel", "achieved": alg, "peak": peak, "unit": "TFLOP/s",
+                "frac": alg / peak,
+                "peak_source": "measured DFMA micro-benchmark (libcatapult_probe.so)" if peak_fp64 else
                 "nominal 148 SM x 64 DFMA/clk x 1.965 GHz",
-                "traffic": _ncu_traffic(model, cnt[6] / max(1, args.steps)),
-                "flops_per_rhs_eval": FLOPS_PER_EVAL[model], "rhs_evals_per_launch": cnt[6] / max(1, args.steps),
+                "flops_per_rhs_eval": ALG_FLOPS_PER_EVAL[model], "flops_per_attempt": ALG_FLOPS_PER_ATTEMPT,
+                "executed": {"achieved": exe, "frac": exe / peak, "flops_per_rhs_eval": EXEC_FLOPS_PER_EVAL[model],
+                             "note": "the kernel's own arithmetic (63-FMA Horner per quantity, no Lagrange basis)"},
+                "traffic": dram_b * evals_per_launch if dram_b else None,
+                "traffic_source": "profiles/r2_traffic_v6c.csv (committed ncu --set full capture, bytes per evaluation) "
+                                  "x the evaluations of one timed launch" if dram_b else None,
+                "rhs_evals_per_launch": evals_per_launch,
                 "launch_ms": sum(trace_ms) / max(1, len(trace_ms)),
                 "trace_share_of_step": sum(trace_ms) / ms,
-                "l2": {"algorithmic_bytes_per_rhs_eval": BYTES_PER_EVAL[model],
-                       "achieved_gbs": alg_bytes / trace_s / 1e9,
+                "cell_fetches_per_rhs_eval": cnt[7] / max(1.0, cnt[6]),
+                "blocking_fetches_per_rhs_eval": cnt[8] / max(1.0, cnt[6]),
+                "slot_efficiency": cnt[6] / max(1.0, 32.0 * cnt[9]),
+                "hbm": {"gbs": dram_b * cnt[6] / trace_s / 1e9 if dram_b else None, "peak_gbs": measured_peaks().get("hbm_gbs")},
+                "l2": {"bytes_per_rhs_eval": l2_b, "algorithmic_bytes_per_rhs_eval":
+                       BYTES_PER_CELL_VISIT[model] * cnt[7] / max(1.0, cnt[6]),
+                       "gbs": l2_b * cnt[6] / trace_s / 1e9 if l2_b else None,
                        "peak_gbs": (l2_bw / 1e9) if l2_bw else None,
-                       "frac": (alg_bytes / trace_s / l2_bw) if l2_bw else None,
-                       "note": "coefficient bytes touched per evaluation / measured L2 read bandwidth"},
-                "hbm_peak_gbs": _measured_peaks().get("hbm_gbs")}
+                       "frac": (l2_b * cnt[6] / trace_s / l2_bw) if (l2_b and l2_bw) else None}}
 
     # ---- end to end: HOST buffers, H2D + D2H inside the timed region, same windows continuing --------
     e2e = None
-    if args.e2e_steps > 0:
+    e2e_steps = args.steps if args.e2e_steps < 0 else args.e2e_steps
+    if e2e_steps > 0:
         f = K.catapult_field_build(fd, d_nodes)
         host = {}
         for k in ("x", "t", "dt", "mu", "status", "nacc", "nrej", "counters"):
             t = state[k]
-            dt_ = {torch.int32: torch.int32, torch.int64: torch.int64}.get(t.dtype, t.dtype)
-            pin = torch.empty(t.shape, dtype=dt_, pin_memory=True)
+            pin = torch.empty(t.shape, dtype=t.dtype, pin_memory=True)
             pin.copy_(t)
             host[k] = pin.numpy()
         host["nacc"] = host["nacc"].view(np.uint32)
         host["nrej"] = host["nrej"].view(np.uint32)
         host["counters"] = host["counters"].view(np.uint64)
-        c0 = host["counters"].copy()
         h2d = sum(host[k].nbytes for k in host)
         d2h = h2d
         barrier()
@@ -322,16 +396,48 @@ def main():
         c0 = host["counters"].copy()
         barrier()
         t0 = time.perf_counter()
-        for j in range(j0 + 1, j0 + 1 + args.e2e_steps):
+        for j in range(j0 + 1, j0 + 1 + e2e_steps):
             K.catapult_trace_continue_host(f, dict(pd, T=(j + 1) * args.window), host)
             _loss = float(np.mean(host["status"] == 1))      # the step's result, read on the host
         torch.cuda.synchronize()
         dt_e2e = time.perf_counter() - t0
         acc_e2e = float(host["counters"][0] - c0[0])
-        dt_e2e, (acc_e2e,) = reduce_over_ranks(dt_e2e, [acc_e2e], world, "cuda")
+        dt_e2e, (acc_e2e,) = S.reduce_timing(dt_e2e, [acc_e2e], device="cuda")
         e2e = {"value": acc_e2e / dt_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-               "steps": args.e2e_steps, "ms_per_step": 1e3 * dt_e2e / args.e2e_steps,
+               "steps": e2e_steps, "ms_per_step": 1e3 * dt_e2e / e2e_steps,
                "api": "catapult_trace_continue_host (pinned host buffers)"}
+        f.destroy()
+        K.catapult_release_host_cache()
+
+    # ---- job leg: t = 0 -> the config's T in ONE launch (population thins, tail under-filled) ----------
+    job = None
+    if args.job_particles != 0:
+        nj = npart if args.job_particles < 0 else min(args.job_particles, npart)
+        Tj = args.job_T if args.job_T > 0 else W.FULL_T[cfg_idx]
+        f = K.catapult_field_build(fd, d_nodes)
+        xj = d_x[:, :nj].contiguous()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        g = K.catapult_trace(f, dict(pd, T=Tj), xj)
+        e1.record()
+        barrier()
+        job_s = e0.elapsed_time(e1) * 1e-3
+        c = g["counters"].cpu().numpy().astype(np.float64)
+        ej = K.catapult_estimate(0, d_status=g["status"])
+        job_s_all, (jacc, jatt, jev, jrounds, jn) = S.reduce_timing(job_s, [c[0], c[0] + c[1], c[6], c[9], nj], device="cuda")
+        jloss = S.reduce_estimate(ej[2], ej[3], nj, device="cuda")
+        ts = g["tstop"][g["status"] == 1].cpu().numpy()
+        edges = Tj * np.array([0.0, 1e-3, 3e-3, 1e-2, 3e-2, 0.1, 0.3, 1.0])
+        job = {"particles": int(jn), "T_s": Tj, "seconds": job_s_all,
+               "particles_to_T_per_s": jn / job_s_all, "accepted_steps_per_s": jacc / job_s_all,
+               "rhs_evals_per_s": jev / job_s_all, "loss_fraction": jloss[0], "loss_fraction_se": jloss[1],
+               "rejected_share_of_attempts": 1.0 - jacc / max(1.0, jatt),
+               "slot_efficiency": jev / max(1.0, 32.0 * jrounds),
+               "resident_slots": 32 * blocks, "gpu_launches": KERNELS_PER_STEP["catapult_trace"],
+               "loss_time_histogram": {"edges_s": edges.tolist(), "counts_rank0": np.histogram(ts, bins=edges)[0].tolist()},
+               "note": "one catapult_trace launch from t = 0; slot_efficiency = evaluations / (32 x block rounds): the share "
+                       "of slot-rounds doing useful work (idle lanes at refill and in the under-filled tail lower it)"}
         f.destroy()
 
     # ---- CPU oracle beside it (rank 0, N = 1 only) ---------------------------------------------------
@@ -353,40 +459,19 @@ def main():
                        "l2_policy": "inputs larger than L2 (512 MiB tables, 126 MB L2)" if table_bytes > (126 << 20)
                        else "tables fit in L2 (resident by design)",
                        "launch": {"blocks": blocks, "threads": threads},
-                       "parallelism": f"dp{world} (one ensemble per GPU, no data-path collective)"},
+                       "parallelism": f"dp{world} (one ensemble of {npart * world} particles split by interleaved "
+                                      "index, tables replicated, one 24-byte all-reduce of the estimate)"},
             "attempted_steps_per_s": att_all / (ms_all * 1e-3),
             "rhs_evals_per_s": evals_all / (ms_all * 1e-3),
             "particle_windows_per_s": world * npart * args.steps / (ms_all * 1e-3),
-            "loss_fraction_so_far": loss_fraction, "particles_alive": alive,
-            "clocks": clocks, "e2e": e2e, "gpu_launches": 4 * args.steps,
-            "roofline": roof, "cpu_baseline": cpu,
+            "particles_to_T_per_s": job["particles_to_T_per_s"] if job else None,
+            "loss_fraction_so_far": loss_fraction, "loss_fraction_se": loss_se, "particles_alive": alive,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches["n"],
+            "roofline": roof, "full_job": job, "cpu_baseline": cpu,
         }
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
-
-
-def _ncu_traffic(model: str, evals_per_launch: float):
-    """DRAM bytes of one trace launch: `dram__bytes_read.sum + dram__bytes_write.sum` per right-hand-side
-    evaluation of the committed `ncu --set full` capture (profiles/r1_traffic_v5.md; cfg4 recipe) times the
-    evaluations of one timed launch.  None for the models that were not captured."""
-    if model != "boozer_saw":
-        return None
-    try:
-        for line in open(os.path.join(ROOT, "profiles", "r1_traffic_v5.csv")):
-            f = line.strip().split(",")
-            if f[0] == "dram_bytes_per_rhs_eval":
-                return float(f[1]) * evals_per_launch
-    except Exception:
-        pass
-    return None
-
-
-def _measured_peaks() -> dict:
-    try:
-        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-    except Exception:
-        return {}
 
 
 if __name__ == "__main__":

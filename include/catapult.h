@@ -204,8 +204,9 @@ catapult_status catapult_step_once(const catapult_field *f, const catapult_trace
 
 /* ---- estimate (Eq. 2) ----------------------------------------------------------
  * g_kind 0: g = 1[status == LOST] (integer count, exact); 1: g = t_stop; 2: g = d_g_user.
- * d_out[3] (device, required) = { mean, standard error sqrt((sum g^2/n - mean^2)/(n-1)), sum g }.
- * Deterministic fixed-order tree.  If h_out != NULL the three doubles are also copied to the host
+ * d_out[4] (device, required) = { mean, standard error sqrt((sum g^2/n - mean^2)/(n-1)), sum g, sum g^2 }:
+ * the two sums (with n) are what a particle-sharded run reduces over its ranks (24 bytes).
+ * Deterministic fixed-order tree.  If h_out != NULL the four doubles are also copied to the host
  * and the stream is synchronised. */
 catapult_status catapult_estimate(int32_t g_kind, int64_t n, const int32_t *d_status,
                                   const double *d_tstop, const double *d_g_user, double *d_out,

@@ -358,12 +358,12 @@ def catapult_step_once(f: Field, pd: dict, d_x, d_t, d_h):
 
 
 def catapult_estimate(g_kind: int, d_status=None, d_tstop=None, d_g_user=None, to_host: bool = True):
-    """Returns (mean, standard error, sum) -- numpy[3] when to_host else a CUDA tensor."""
+    """Returns (mean, standard error, sum g, sum g^2) -- numpy[4] when to_host else a CUDA tensor."""
     torch = _torch()
     ref = d_status if d_status is not None else (d_tstop if d_tstop is not None else d_g_user)
     n = ref.shape[0]
-    out = torch.empty(3, dtype=torch.float64, device=ref.device)
-    h = np.zeros(3) if to_host else None
+    out = torch.empty(4, dtype=torch.float64, device=ref.device)
+    h = np.zeros(4) if to_host else None
     _check(load().catapult_estimate(g_kind, n, _ptr(d_status, torch.int32, True), _ptr(d_tstop, torch.float64, True),
                                     _ptr(d_g_user, torch.float64, True), _ptr(out), _hptr(h, np.float64), _stream()))
     return h if to_host else out

@@ -553,7 +553,7 @@ catapult_status catapult_estimate(int32_t g_kind, int64_t n, const int32_t* d_st
   catapult_status st = launch_estimate(g_kind, n, d_status, d_tstop, d_g_user, d_out, (cudaStream_t)stream);
   if (st != CATAPULT_OK) return st;
   if (h_out) {
-    CATAPULT_CUDA_TRY(cudaMemcpyAsync(h_out, d_out, 3 * sizeof(double), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CATAPULT_CUDA_TRY(cudaMemcpyAsync(h_out, d_out, 4 * sizeof(double), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
     CATAPULT_CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
   }
   return CATAPULT_OK;

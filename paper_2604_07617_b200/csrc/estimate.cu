@@ -58,6 +58,7 @@ __global__ void estimate_final_kernel(long long n, int nblocks, const double* __
   out[0] = mean;
   out[1] = sqrt(var);
   out[2] = sum;
+  out[3] = sum2;
 }
 
 catapult_status launch_estimate(int g_kind, int64_t n, const int* d_status, const double* d_tstop, const double* d_g,

@@ -626,7 +626,9 @@ def test_estimate_parity(K, oracle):
             want = oracle.estimate(kind, status=status, tstop=tstop, g_user=tstop ** 2)
             if kind == 0:
                 assert got[2] == want[2] and got[0] == want[0]        # integer count: exact
-            assert np.allclose(got, want, rtol=1e-12, atol=1e-300)
+            assert np.allclose(got[:3], want, rtol=1e-12, atol=1e-300)
+            g_ = (status == 1).astype(float) if kind == 0 else (tstop if kind == 1 else tstop ** 2)
+            assert abs(got[3] - np.sum(g_ * g_)) <= 1e-12 * max(np.sum(g_ * g_), 1e-300)
     with pytest.raises(K.CatapultError):
         K.catapult_estimate(0, d_status=None, d_tstop=_dev(np.zeros(3)))
 

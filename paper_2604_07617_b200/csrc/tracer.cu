@@ -711,8 +711,10 @@ static catapult_status trace_dispatch(const TraceConst& tc, const TraceArgs& a, 
 }
 
 catapult_status launch_trace(const TraceConst& tc, const TraceArgs& a, int model, int mode, cudaStream_t s) {
-#ifndef CATAPULT_BOOZER_SPLIT
+#if defined(CATAPULT_BOOZER_LANE)
   if (model != MODEL_CART) return launch_trace_lane(tc, a, model, mode, s);
+#elif !defined(CATAPULT_BOOZER_SPLIT)
+  if (model != MODEL_CART) return launch_trace_pair(tc, a, model, mode, s);
 #endif
   switch (mode) {
     case MODE_ADAPTIVE: return trace_dispatch<MODE_ADAPTIVE>(tc, a, model, s);
@@ -722,8 +724,10 @@ catapult_status launch_trace(const TraceConst& tc, const TraceArgs& a, int model
 }
 
 catapult_status trace_launch_shape(int model, int64_t n, int* blocks, int* threads) {
-#ifndef CATAPULT_BOOZER_SPLIT
+#if defined(CATAPULT_BOOZER_LANE)
   if (model != MODEL_CART) return trace_lane_shape(model, n, blocks, threads);
+#elif !defined(CATAPULT_BOOZER_SPLIT)
+  if (model != MODEL_CART) return trace_pair_shape(model, n, blocks, threads);
 #endif
   switch (model) {
     case MODEL_BOOZER_VAC: return trace_shape<MODEL_BOOZER_VAC, MODE_ADAPTIVE>(n, blocks, threads);

@@ -199,5 +199,8 @@ __device__ __forceinline__ void eval_physics(const TraceConst& tc, const double 
 // tracer_lane.cu
 catapult_status launch_trace_lane(const TraceConst& tc, const TraceArgs& a, int model, int mode, cudaStream_t s);
 catapult_status trace_lane_shape(int model, int64_t n, int* blocks, int* threads);
+// tracer_pair.cu
+catapult_status launch_trace_pair(const TraceConst& tc, const TraceArgs& a, int model, int mode, cudaStream_t s);
+catapult_status trace_pair_shape(int model, int64_t n, int* blocks, int* threads);
 
 }  // namespace catapult

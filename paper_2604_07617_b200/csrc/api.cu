@@ -274,8 +274,8 @@ static catapult_status run_trace(const catapult_field* f, const catapult_trace_p
   if (st != CATAPULT_OK) return st;
   if (a.n == 0) return CATAPULT_OK;
   unsigned long long* queue = nullptr;
-  CATAPULT_CUDA_TRY(cudaMallocAsync((void**)&queue, sizeof(unsigned long long), s));
-  cudaError_t e = cudaMemsetAsync(queue, 0, sizeof(unsigned long long), s);
+  CATAPULT_CUDA_TRY(cudaMallocAsync((void**)&queue, TRACE_SCRATCH_BYTES, s));
+  cudaError_t e = cudaMemsetAsync(queue, 0, TRACE_SCRATCH_BYTES, s);
   if (e != cudaSuccess) {
     cudaFreeAsync(queue, s);
     return cuda_fail(e, "cudaMemsetAsync(queue)");
@@ -531,8 +531,8 @@ catapult_status catapult_step_once(const catapult_field* f, const catapult_trace
   a.kall = d_k;
   cudaStream_t s = (cudaStream_t)stream;
   unsigned long long* queue = nullptr;
-  CATAPULT_CUDA_TRY(cudaMallocAsync((void**)&queue, sizeof(unsigned long long), s));
-  cudaError_t e = cudaMemsetAsync(queue, 0, sizeof(unsigned long long), s);
+  CATAPULT_CUDA_TRY(cudaMallocAsync((void**)&queue, TRACE_SCRATCH_BYTES, s));
+  cudaError_t e = cudaMemsetAsync(queue, 0, TRACE_SCRATCH_BYTES, s);
   if (e != cudaSuccess) {
     cudaFreeAsync(queue, s);
     return cuda_fail(e, "cudaMemsetAsync(queue)");

@@ -43,7 +43,8 @@ struct TraceArgs {
   unsigned* nacc;      // nullable
   unsigned* nrej;      // nullable
   unsigned long long* counters;  // nullable, CATAPULT_NCOUNTERS entries
-  unsigned long long* queue;     // work counter, zero at launch
+  unsigned long long* queue;     // TRACE_SCRATCH_BYTES, zero at launch: the work counter, then one int per SM
+                                 // (how many blocks of the launch have started there)
   int resume;     // 1: continue from (t,dt,mu,status) arrays
   int init_only;  // 1: only fill (t,dt,mu,status)
   // scripted replay (catapult_trace_scripted): step sizes are read instead of controlled
@@ -52,6 +53,8 @@ struct TraceArgs {
   int script_len;
   double* kall;            // step-once hook: [7][4][n] stage derivatives
 };
+
+constexpr size_t TRACE_SCRATCH_BYTES = 8 + 4 * 1024;
 
 void set_error(const std::string& msg);
 catapult_status cuda_fail(cudaError_t e, const char* what);

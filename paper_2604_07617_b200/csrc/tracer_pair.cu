@@ -54,8 +54,8 @@ struct PairTraits {
   static constexpr size_t OFF_PART = OFF_KS + (size_t)7 * 4 * NS * 8;  // double2 [4 planes][2][NS]: plane values
   static constexpr size_t OFF_W = OFF_PART + (size_t)8 * NS * 16;     // double [2][NS]: wFIRST, wSECOND
   static constexpr size_t OFF_G = OFF_W + (size_t)2 * NS * 8;         // int2 [2 parities][NS]: (redo cell, next cell)
-  static constexpr size_t OFF_G2 = OFF_G + (size_t)2 * NS * 8;        // int [NS]: next cell after accept / reject
-  static constexpr size_t OFF_REQ = OFF_G2 + (size_t)NS * 4;          // int [NS]: request word
+  static constexpr size_t OFF_G2 = OFF_G + (size_t)2 * NS * 8;        // int2 [NS]: after accept / reject: (next cell, cell at the end of the next step)
+  static constexpr size_t OFF_REQ = OFF_G2 + (size_t)NS * 8;          // int [NS]: request word
   static constexpr size_t SMEM_BYTES = OFF_REQ + (size_t)NS * 4;
   static_assert(2 * (SMEM_BYTES + 1024) <= 233472, "two blocks per SM: 228 KB of shared memory");
 };
@@ -198,7 +198,7 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
   const double* wbuf = reinterpret_cast<const double*>(smem + PT::OFF_W) + slot;
   const volatile int* reqbuf = reinterpret_cast<const volatile int*>(smem + PT::OFF_REQ) + slot;
   const volatile long long* gbuf = reinterpret_cast<const volatile long long*>(smem + PT::OFF_G) + slot;
-  const volatile int* g2buf = reinterpret_cast<const volatile int*>(smem + PT::OFF_G2) + slot;
+  const volatile long long* g2buf = reinterpret_cast<const volatile long long*>(smem + PT::OFF_G2) + slot;
 
   for (;;) {
     pbar_sync(bar0 + PB_REQ);
@@ -235,8 +235,16 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
     if (active && next_cell >= 0 && next_cell != pc.cached) pair_fetch(table, pc, creg, next_cell);
     if (kind == 5) {  // end of an attempt: the first point of the next one depends on the accept / reject decision
       pbar_sync(bar0 + PB_G2);
-      const int t2 = g2buf[0];
+      const long long g2 = g2buf[0];
+      const int t2 = (int)g2, far = (int)(g2 >> 32);
       if (active && t2 >= 0 && t2 != pc.cached) pair_fetch(table, pc, creg, t2);
+      // the cell in which the next attempt is expected to end: towards L2 now (30 % of the fetches come from
+      // HBM otherwise, and a warp waits for its slowest lane)
+      if (active && far >= 0 && far != pc.cached) {
+        const char* line = reinterpret_cast<const char*>(table + (long long)far * PT::NCOEF);
+#pragma unroll
+        for (int l = 0; l < PT::NCOEF * 8 / 128; ++l) asm volatile("prefetch.global.L2 [%0];" ::"l"(line + 128 * l));
+      }
     }
   }
 }
@@ -371,12 +379,21 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
   extern __shared__ __align__(16) unsigned char smem[];
   const int lane = threadIdx.x & 31;
   const int warp = threadIdx.x >> 5;
-  // warps 0, 1: scalar warps of pairs 0, 1; warps 2, 3: their contraction warps (every scheduler of the SM hosts
-  // one warp of this block and one of the other resident block)
+  // A block's warps w and w ^ 2 form pair w & 1.  Which of the two is the scalar warp alternates between the two
+  // blocks resident on an SM (counted per SM as they start), so that each of the SM's four schedulers hosts one
+  // scalar and one contraction warp and the contraction's DFMA load is spread over all four FP64 pipes.
+  __shared__ int flip_s;
+  if (threadIdx.x == 0) {
+    unsigned smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    flip_s = (int)(atomicAdd(reinterpret_cast<unsigned*>(a.queue + 1) + (smid & 1023u), 1u) & 1u);
+  }
+  __syncthreads();
+  const int flip = flip_s;
   const int pair = warp & 1;
   const int slot = pair * 32 + lane;
   const int bar0 = 1 + 6 * pair;
-  if (warp >= 2) {
+  if ((warp >> 1) != flip) {
     contraction_warp(tc, smem, slot, bar0);
     return;
   }
@@ -608,7 +625,7 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
         // the decision goes to the contraction warp at once: the cell of the next attempt's first point, a fifth
         // of the next step length beyond the new start point (accepted: the end point; rejected: the old start
         // point)
-        int target = -1;
+        int target = -1, far = -1;
         if (MODE != MODE_STEP_ONCE && stepping) {
           double hn = h;
           if (MODE == MODE_ADAPTIVE) {
@@ -617,6 +634,7 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
           }
           const float fr = 0.2f * __fdividef((float)hn, (float)h);
           target = guess_cell<MODEL>(tc.f, pos, base, accepted ? fr : fr - 1.0f);
+          far = guess_cell<MODEL>(tc.f, pos, base, accepted ? 5.0f * fr : 5.0f * fr - 1.0f);
           sr.n_load += (unsigned)(target != sr.held);
           sr.held = target;
           if (accepted) {
@@ -624,7 +642,7 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
             for (int d = 0; d < 3; ++d) base[d] = pos[d];
           }
         }
-        reinterpret_cast<int*>(smem + PT::OFF_G2)[slot] = target;
+        reinterpret_cast<int2*>(smem + PT::OFF_G2)[slot] = make_int2(target, far);
         __syncwarp();
         pbar_arrive(bar0 + PB_G2);
       }

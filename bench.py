@@ -56,10 +56,13 @@ UNIT = "accepted steps/s"
 # ~150 flops of stage / error algebra.  `roofline.achieved` and `roofline.frac` use these.
 ALG_FLOPS_PER_EVAL = {"boozer_vac": 4 * 168 + 30 + 100, "boozer_saw": 4 * 168 + 30 + 150, "cart": 7 * 168 + 30 + 120}
 ALG_FLOPS_PER_ATTEMPT = 150
-# EXECUTED work of trace_kernel (its own arithmetic: 63-FMA Horner per quantity in the monomial basis, no Lagrange
-# basis; the scalar warp's and the stage sums' DFMA / DMUL / DADD per evaluation from the ncu instruction mix of the
-# committed capture, profiles/r2_ncu_trace_v6c.md).  `roofline.executed` uses these; stage algebra included.
-EXEC_FLOPS_PER_EVAL = {"boozer_vac": 4 * 126 + 215, "boozer_saw": 4 * 126 + 307, "cart": 7 * 126 + 260}
+# EXECUTED work of the tracer kernels (their own arithmetic: 63-FMA Horner per quantity in the monomial basis, no
+# Lagrange basis; the scalar warp's and the stage sums' DFMA / DMUL / DADD per evaluation from the ncu instruction mix
+# of the committed capture, profiles/r2_ncu_trace_pair.md: 391 DFMA + 75 DMUL + 22 DADD thread instructions per
+# evaluation, lanes without a particle included).  `roofline.executed` uses these; stage algebra included.
+EXEC_FLOPS_PER_EVAL = {"boozer_vac": 4 * 126 + 275, "boozer_saw": 4 * 126 + 375, "cart": 7 * 126 + 260}
+# particle slots served by one thread block (tracer_pair.cu: two warp pairs; tracer.cu: one scalar warp)
+SLOTS_PER_BLOCK = {"boozer_vac": 64, "boozer_saw": 64, "cart": 32}
 BYTES_PER_CELL_VISIT = {"boozer_vac": 4 * 512, "boozer_saw": 4 * 512, "cart": 7 * 512}
 KERNELS_PER_STEP = {"catapult_field_build": 1, "catapult_trace_continue": 1, "catapult_trace": 1, "catapult_estimate": 2}
 
@@ -137,7 +140,7 @@ def oracle_sample(cfg, window: float, nsample: int, nthreads: int = 0) -> dict:
     r = O.trace(f, p, x0, nthreads)
     dt = time.perf_counter() - t0
     acc = int(r["nacc"].sum())
-    return dict(value=acc / dt, seconds=dt, accepted=acc, attempts=acc + int(r["nrej"].sum()),
+    return dict(value=acc / dt, seconds=dt, accepted=acc, attempts=acc + int(r["nrej"].sum()), status=r["status"],
                 cores=nthreads if nthreads > 0 else O.max_threads(),
                 sample=f"first {x0.shape[1]} particles of {cfg['name']} over [0, {window:g}] s")
 
@@ -188,11 +191,11 @@ def spawn_ranks(args) -> int:
 
 def committed_capture(model: str) -> dict:
     """Per-evaluation DRAM / L2 bytes of trace_kernel from the committed `ncu --set full` capture of this kernel
-    (profiles/r2_traffic_v6c.csv; the command is in the .md beside it).  bench.py does not run ncu: the traffic
+    (profiles/r2_traffic_pair.csv; the command is in the .md beside it).  bench.py does not run ncu: the traffic
     it reports is that capture's per-evaluation figure times the evaluations of its own timed launches."""
     out = {}
     try:
-        for line in open(os.path.join(ROOT, "profiles", "r2_traffic_v6c.csv")):
+        for line in open(os.path.join(ROOT, "profiles", "r2_traffic_pair.csv")):
             f = line.strip().split(",")
             if len(f) >= 3 and f[0] == model:
                 out[f[1]] = float(f[2])
@@ -224,6 +227,9 @@ def main():
     ap.add_argument("--job-particles", type=int, default=65536,
                     help="particles of the full-T job leg (0 = skip, -1 = the whole ensemble)")
     ap.add_argument("--job-T", type=float, default=0.0, help="end time of the job leg (0 = the config's own T)")
+    ap.add_argument("--job-oracle", type=int, default=0, help="fidelity leg of the sweep (PAPER.md:98-102): the oracle traces "
+                    "the first N particles of the job leg to the same end time; loss fractions and per-particle loss "
+                    "flags are compared (0 = skip)")
     ap.add_argument("--cpu-particles", type=int, default=2048, help="oracle sample for cpu_baseline (0 = skip)")
     ap.add_argument("--ref-particles", type=int, default=1024)
     ap.add_argument("--no-peaks", action="store_true")
@@ -351,7 +357,7 @@ def main():
         cap = committed_capture(model)
         evals_per_launch = cnt[6] / max(1, args.steps)
         dram_b, l2_b = cap.get("dram_bytes_per_rhs_eval"), cap.get("l2_bytes_per_rhs_eval")
-        roof = {"bound": "alu", "kernel": "trace_kernel", "achieved": alg, "peak": peak, "unit": "TFLOP/s",
+        roof = {"bound": "alu", "kernel": "trace_kernel" if model == "cart" else "trace_pair_kernel", "achieved": alg, "peak": peak, "unit": "TFLOP/s",
                 "frac": alg / peak,
                 "peak_source": "measured DFMA micro-benchmark (libcatapult_probe.so)" if peak_fp64 else
                 "nominal 148 SM x 64 DFMA/clk x 1.965 GHz",
@@ -359,7 +365,7 @@ def main():
                 "executed": {"achieved": exe, "frac": exe / peak, "flops_per_rhs_eval": EXEC_FLOPS_PER_EVAL[model],
                              "note": "the kernel's own arithmetic (63-FMA Horner per quantity, no Lagrange basis)"},
                 "traffic": dram_b * evals_per_launch if dram_b else None,
-                "traffic_source": "profiles/r2_traffic_v6c.csv (committed ncu --set full capture, bytes per evaluation) "
+                "traffic_source": "profiles/r2_traffic_pair.csv (committed ncu --set full capture, bytes per evaluation) "
                                   "x the evaluations of one timed launch" if dram_b else None,
                 "rhs_evals_per_launch": evals_per_launch,
                 "launch_ms": sum(trace_ms) / max(1, len(trace_ms)),
@@ -434,10 +440,21 @@ def main():
                "rhs_evals_per_s": jev / job_s_all, "loss_fraction": jloss[0], "loss_fraction_se": jloss[1],
                "rejected_share_of_attempts": 1.0 - jacc / max(1.0, jatt),
                "slot_efficiency": jev / max(1.0, 32.0 * jrounds),
-               "resident_slots": 32 * blocks, "gpu_launches": KERNELS_PER_STEP["catapult_trace"],
+               "resident_slots": SLOTS_PER_BLOCK[model] * blocks, "gpu_launches": KERNELS_PER_STEP["catapult_trace"],
                "loss_time_histogram": {"edges_s": edges.tolist(), "counts_rank0": np.histogram(ts, bins=edges)[0].tolist()},
                "note": "one catapult_trace launch from t = 0; slot_efficiency = evaluations / (32 x block rounds): the share "
                        "of slot-rounds doing useful work (idle lanes at refill and in the under-filled tail lower it)"}
+        if rank == 0 and world == 1 and args.job_oracle > 0:
+            # the CPU oracle on the first particles of the same job (same field, tolerance and end time): what the
+            # paper's fidelity axis measures (loss fraction against cells per dimension and tolerance)
+            no = min(args.job_oracle, nj)
+            r = oracle_sample(dict(cfg, x0=cfg["x0"][:, :no]), Tj, no)
+            lost_o = r["status"] == 1
+            lost_g = (g["status"][:no] == 1).cpu().numpy()
+            job["oracle"] = {"particles": no, "seconds": r["seconds"], "cores": r["cores"],
+                             "loss_fraction_oracle": float(lost_o.mean()), "loss_fraction_gpu_same_particles": float(lost_g.mean()),
+                             "loss_flags_agree": float((lost_o == lost_g).mean()),
+                             "binomial_sigma": float(math.sqrt(max(lost_o.mean() * (1 - lost_o.mean()), 1e-12) / no))}
         f.destroy()
 
     # ---- CPU oracle beside it (rank 0, N = 1 only) ---------------------------------------------------

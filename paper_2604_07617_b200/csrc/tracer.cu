@@ -1,8 +1,10 @@
-// Persistent fp64 DP5 guiding-centre tracer: warp-specialised, pipelined along the interpolation axes.
+// Persistent fp64 DP5 guiding-centre tracer: warp-specialised, pipelined along the interpolation axes.  This
+// kernel serves the cylindrical model (7 tabulated quantities, 3.5 KiB of coefficients per cell); the Boozer models
+// (4 quantities) are served by the warp-pair kernel of tracer_pair.cu, which launch_trace() dispatches to.
 //
 // What is computed is PAPER.md:57-61 (DESIGN.md sections 1-2); the launch shape is this library's own.
 //
-// A block serves 32 particle slots with NQ + 1 warps (NQ = tabulated quantities: 4 Boozer, 7 cylindrical):
+// A block serves 32 particle slots with NQ + 1 warps (NQ = tabulated quantities):
 //   * the SCALAR warp: lane l owns particle slot l -- state, DP5 stage states, cell locate, the guiding-centre
 //     physics, error norm, controller, stop test and refill.  One warp instruction advances 32 particles.
 //   * NQ CONTRACTION warps: lane l of warp q owns the 64 tricubic coefficients of quantity q of slot l's
@@ -26,12 +28,6 @@
 
 namespace catapult {
 
-#ifndef CATAPULT_MINB_BOOZER
-#define CATAPULT_MINB_BOOZER 4
-#endif
-#ifndef CATAPULT_MINB_CART
-#define CATAPULT_MINB_CART 2
-#endif
 
 
 template <int MODEL>
@@ -40,7 +36,7 @@ struct TraceTraits {
   static constexpr int NQ = CART ? CATAPULT_NQUANT_CYL : CATAPULT_NQUANT_BOOZER;
   static constexpr int NT = 32 * (NQ + 1);   // threads per block
   static constexpr int NCT = 32 * NQ;        // contraction threads per block
-  static constexpr int MINB = CART ? CATAPULT_MINB_CART : CATAPULT_MINB_BOOZER;
+  static constexpr int MINB = CART ? 2 : 4;  // resident blocks per SM
   // A contraction thread keeps the first 32 stored coefficients of its (cell, quantity) block (LAST-power 0, 1:
   // gc_device.cuh) in registers and the other 32 in a private run of shared memory: 256 bytes + 16 bytes of
   // padding, so that the 8 lanes of a quarter warp reading 16 bytes each at the same offset of their runs hit 8
@@ -703,19 +699,12 @@ static catapult_status trace_launch(const TraceConst& tc, const TraceArgs& a, cu
 template <int MODE>
 static catapult_status trace_dispatch(const TraceConst& tc, const TraceArgs& a, int model, cudaStream_t s) {
   if (a.n == 0) return CATAPULT_OK;
-  switch (model) {
-    case MODEL_BOOZER_VAC: return trace_launch<MODEL_BOOZER_VAC, MODE>(tc, a, s);
-    case MODEL_BOOZER_SAW: return trace_launch<MODEL_BOOZER_SAW, MODE>(tc, a, s);
-    default: return trace_launch<MODEL_CART, MODE>(tc, a, s);
-  }
+  (void)model;  // the Boozer models are served by tracer_pair.cu
+  return trace_launch<MODEL_CART, MODE>(tc, a, s);
 }
 
 catapult_status launch_trace(const TraceConst& tc, const TraceArgs& a, int model, int mode, cudaStream_t s) {
-#if defined(CATAPULT_BOOZER_LANE)
-  if (model != MODEL_CART) return launch_trace_lane(tc, a, model, mode, s);
-#elif !defined(CATAPULT_BOOZER_SPLIT)
-  if (model != MODEL_CART) return launch_trace_pair(tc, a, model, mode, s);
-#endif
+  if (model != MODEL_CART) return launch_trace_pair(tc, a, model, mode, s);  // tracer_pair.cu
   switch (mode) {
     case MODE_ADAPTIVE: return trace_dispatch<MODE_ADAPTIVE>(tc, a, model, s);
     case MODE_SCRIPT: return trace_dispatch<MODE_SCRIPT>(tc, a, model, s);
@@ -724,16 +713,8 @@ catapult_status launch_trace(const TraceConst& tc, const TraceArgs& a, int model
 }
 
 catapult_status trace_launch_shape(int model, int64_t n, int* blocks, int* threads) {
-#if defined(CATAPULT_BOOZER_LANE)
-  if (model != MODEL_CART) return trace_lane_shape(model, n, blocks, threads);
-#elif !defined(CATAPULT_BOOZER_SPLIT)
   if (model != MODEL_CART) return trace_pair_shape(model, n, blocks, threads);
-#endif
-  switch (model) {
-    case MODEL_BOOZER_VAC: return trace_shape<MODEL_BOOZER_VAC, MODE_ADAPTIVE>(n, blocks, threads);
-    case MODEL_BOOZER_SAW: return trace_shape<MODEL_BOOZER_SAW, MODE_ADAPTIVE>(n, blocks, threads);
-    default: return trace_shape<MODEL_CART, MODE_ADAPTIVE>(n, blocks, threads);
-  }
+  return trace_shape<MODEL_CART, MODE_ADAPTIVE>(n, blocks, threads);
 }
 
 }  // namespace catapult

@@ -1,5 +1,5 @@
-// Pieces shared by the two tracer kernels (tracer_lane.cu: one thread per particle, Boozer models;
-// tracer.cu: warp-specialised, cylindrical model): the Dormand-Prince tableau, the asynchronous-copy helpers,
+// Pieces shared by the two tracer kernels (tracer_pair.cu: warp pairs, Boozer models; tracer.cu: one scalar warp +
+// one contraction warp per quantity, cylindrical model): the Dormand-Prince tableau, the asynchronous-copy helpers,
 // the next-cell guess and the guiding-centre right-hand sides (R1-R3).
 #pragma once
 
@@ -196,9 +196,6 @@ __device__ __forceinline__ void eval_physics(const TraceConst& tc, const double 
   }
 }
 
-// tracer_lane.cu
-catapult_status launch_trace_lane(const TraceConst& tc, const TraceArgs& a, int model, int mode, cudaStream_t s);
-catapult_status trace_lane_shape(int model, int64_t n, int* blocks, int* threads);
 // tracer_pair.cu
 catapult_status launch_trace_pair(const TraceConst& tc, const TraceArgs& a, int model, int mode, cudaStream_t s);
 catapult_status trace_pair_shape(int model, int64_t n, int* blocks, int* threads);

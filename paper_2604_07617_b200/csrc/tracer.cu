@@ -286,6 +286,7 @@ __device__ __forceinline__ void scalar_round(const TraceConst& tc, unsigned char
     unit_power(tc.saw_m, g.ca, g.sa, cm, sm);
     g.sn = fma(sm, cb, cm * sb);
     g.cs = fma(cm, cb, -sm * sb);
+    eval_wave_terms(tc, g);
   }
   // ---- the last coordinate and the cell
   {

@@ -128,7 +128,30 @@ struct EvalGeo {
   double a, inva;                  // Boozer: s, 1/s;  Cartesian: R, 1/R
   double ca, sa;                   // cosine and sine of theta (phi): y0/a, y1/a
   double sn, cs, Phihat, dPhihat;  // wave terms (MODEL_BOOZER_SAW)
+  // ... and what the right-hand side makes of them without the field values (eval_wave_terms)
+  double Phi_psi, Phi_th, al_th, iag, iagG, t2;
 };
+
+// The part of R2 that does not need the interpolated field: computed while the
+// contraction is still running.  Same operations, same order as if written inside eval_physics.
+__device__ __forceinline__ void eval_wave_terms(const TraceConst& tc, EvalGeo& g) {
+  const FieldConst& f = tc.f;
+  const double mm = (double)tc.saw_m, nn = (double)tc.saw_n;
+  const double Phihat = g.Phihat, dPhihat = g.dPhihat, sn = g.sn, cs = g.cs;
+  const double iota = fma(f.iota1, g.a, f.iota0);
+  const double Phi = Phihat * sn;
+  g.Phi_psi = dPhihat * sn * f.invpsi0;
+  g.Phi_th = mm * Phihat * cs;
+  const double Phi_ze = -nn * Phihat * cs;
+  const double kpar = fma(iota, mm, -nn);
+  const double inv_omG = tc.saw_inv_omG;
+  g.al_th = -kpar * g.Phi_th * inv_omG;
+  const double al_t = -kpar * Phihat * cs * f.invG;
+  const double al_psi = -fma(f.iota1 * mm, Phi, kpar * dPhihat * sn) * inv_omG * f.invpsi0;
+  g.iag = fma(-al_psi, f.G, iota);  // iota - alpha_psi G
+  g.iagG = g.iag * f.invG;
+  g.t2 = tc.q * fma(al_t, f.G, fma(g.al_th * f.G, g.Phi_psi, fma(g.iag, g.Phi_th, Phi_ze)));
+}
 
 // DESIGN.md R1-R3 with the interpolated values fv
 template <int MODEL>
@@ -168,24 +191,13 @@ __device__ __forceinline__ void eval_physics(const TraceConst& tc, const double 
       thdot = fma(B_psi, W, iota * vBG);
       vdot = -fma(iota, B_th, B_ze) * mu * B * f.invG;
     } else {
-      const double mm = (double)tc.saw_m, nn = (double)tc.saw_n;
-      const double Phihat = g.Phihat, dPhihat = g.dPhihat, sn = g.sn, cs = g.cs;
-      const double Phi = Phihat * sn;
-      const double Phi_psi = dPhihat * sn * f.invpsi0;
-      const double Phi_th = mm * Phihat * cs;
-      const double Phi_ze = -nn * Phihat * cs;
-      const double kpar = fma(iota, mm, -nn);
-      const double inv_omG = tc.saw_inv_omG;
-      const double al_th = -kpar * Phi_th * inv_omG;
-      const double al_t = -kpar * Phihat * cs * f.invG;
-      const double al_psi = -fma(f.iota1 * mm, Phi, kpar * dPhihat * sn) * inv_omG * f.invpsi0;
+      // the wave's own terms come from eval_wave_terms (the caller has run it for this point)
+      const double Phi_psi = g.Phi_psi, Phi_th = g.Phi_th, al_th = g.al_th, iag = g.iag;
       const double psidot = fma(-B_th, W, fma(al_th, B * vpar, -Phi_th));
       sdot = psidot * f.invpsi0;
-      const double iag = fma(-al_psi, f.G, iota);  // iota - alpha_psi G
-      thdot = fma(B_psi, W, fma(iag * f.invG, vpar * B, Phi_psi));
+      thdot = fma(B_psi, W, fma(g.iagG, vpar * B, Phi_psi));
       const double t1 = tc.M * mu * fma(al_th * B_psi, f.G, fma(B_th, iag, B_ze));
-      const double t2 = tc.q * fma(al_t, f.G, fma(al_th * f.G, Phi_psi, fma(iag, Phi_th, Phi_ze)));
-      vdot = fma(-(B * f.invG * tc.invM), t1 + t2, vpar * invB * fma(B_th, Phi_psi, -B_psi * Phi_th));
+      vdot = fma(-(B * f.invG * tc.invM), t1 + g.t2, vpar * invB * fma(B_th, Phi_psi, -B_psi * Phi_th));
     }
     dy[0] = fma(sdot, g.ca, -thdot * y[1]);
     dy[1] = fma(sdot, g.sa, thdot * y[0]);

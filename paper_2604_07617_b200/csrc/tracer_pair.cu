@@ -50,8 +50,8 @@ struct PairTraits {
   static_assert((STRIP / 16) % 2 == 1, "run length must be an odd number of 16-byte groups");
   static constexpr size_t OFF_COEF = 0;                               // [NS] runs of STRIP bytes
   static constexpr size_t OFF_MBAR = OFF_COEF + (size_t)STRIP * NS;   // uint64 [NS]: one mbarrier per slot
-  static constexpr size_t OFF_KS = OFF_MBAR + 8 * NS;                 // double [7][4][NS]: stage derivatives
-  static constexpr size_t OFF_PART = OFF_KS + (size_t)7 * 4 * NS * 8;  // double2 [4 planes][2][NS]: plane values
+  static constexpr size_t OFF_KS = OFF_MBAR + 8 * NS;                 // double [6][4][NS]: stage derivatives k_1..k_6
+  static constexpr size_t OFF_PART = OFF_KS + (size_t)6 * 4 * NS * 8;  // double2 [4 planes][2][NS]: plane values
   static constexpr size_t OFF_W = OFF_PART + (size_t)8 * NS * 16;     // double [2][NS]: wFIRST, wSECOND
   static constexpr size_t OFF_G = OFF_W + (size_t)2 * NS * 8;         // int2 [2 parities][NS]: (redo cell, next cell)
   static constexpr size_t OFF_G2 = OFF_G + (size_t)2 * NS * 8;        // int2 [NS]: after accept / reject: (next cell, cell at the end of the next step)
@@ -141,33 +141,40 @@ __device__ __forceinline__ void quad_rows(const double (&c)[4][4], double wF, do
 // horner_plane (gc_device.cuh), which every user of the table follows.  The 64 rows are walked with the quantity
 // running fastest (quad_rows: 16 quads, plane a = 3 first); the rows of a quad that live in shared memory are
 // loaded PAIR_AHEAD quads ahead into rotating row buffers; a finished plane goes to the exchange buffer at once.
-__device__ __forceinline__ void pair_contract(const double (&creg)[PairTraits::NREG], unsigned strip_s,
-                                              unsigned part_s, double wS, double wF) {
-  using PT = PairTraits;
-  constexpr int AHEAD = CATAPULT_PAIR_AHEAD;
+struct PairRows {  // rotating row buffers of the contraction: [quad modulo (AHEAD + 1)][quantity][4 coefficients]
+  static constexpr int AHEAD = CATAPULT_PAIR_AHEAD;
   double rb[AHEAD + 1][4][4];
-  auto first_coef = [](int s, int q) {  // quad s = (a, b) descending
+  static __device__ __forceinline__ constexpr int first_coef(int s, int q) {  // quad s = (a, b) descending
     return q * 64 + ((3 - s / 4) * 4 + (3 - s % 4)) * 4;
-  };
-  auto load_quad = [&](int s) {
+  }
+  __device__ __forceinline__ void load_quad(unsigned strip_s, int s) {
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const int g = first_coef(s, q);
-      if (g >= PT::NREG) lds_row(strip_s + (unsigned)(g - PT::NREG) * 8u, rb[s % (AHEAD + 1)][q]);
+      if (g >= PairTraits::NREG) lds_row(strip_s + (unsigned)(g - PairTraits::NREG) * 8u, rb[s % (AHEAD + 1)][q]);
     }
-  };
+  }
+  // the rows the first quads need do not depend on the evaluation point: they can be loaded before it is known
+  __device__ __forceinline__ void preload(unsigned strip_s) {
 #pragma unroll
-  for (int s = 0; s < AHEAD; ++s) load_quad(s);
+    for (int s = 0; s < AHEAD; ++s) load_quad(strip_s, s);
+  }
+};
+
+__device__ __forceinline__ void pair_contract(const double (&creg)[PairTraits::NREG], PairRows& rows,
+                                              unsigned strip_s, unsigned part_s, double wS, double wF) {
+  using PT = PairTraits;
+  constexpr int AHEAD = PairRows::AHEAD;
   double P[4];
 #pragma unroll
   for (int s = 0; s < 16; ++s) {
-    if (s + AHEAD < 16) load_quad(s + AHEAD);
+    if (s + AHEAD < 16) rows.load_quad(strip_s, s + AHEAD);
     double c[4][4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-      const int g = first_coef(s, q);
+      const int g = PairRows::first_coef(s, q);
 #pragma unroll
-      for (int e = 0; e < 4; ++e) c[q][e] = (g < PT::NREG) ? creg[g < PT::NREG ? g + e : 0] : rb[s % (AHEAD + 1)][q][e];
+      for (int e = 0; e < 4; ++e) c[q][e] = (g < PT::NREG) ? creg[g < PT::NREG ? g + e : 0] : rows.rb[s % (AHEAD + 1)][q][e];
     }
     if (s % 4 == 0) quad_rows<true>(c, wF, wS, P);
     else quad_rows<false>(c, wF, wS, P);
@@ -200,7 +207,13 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
   const volatile long long* gbuf = reinterpret_cast<const volatile long long*>(smem + PT::OFF_G) + slot;
   const volatile long long* g2buf = reinterpret_cast<const volatile long long*>(smem + PT::OFF_G2) + slot;
 
+  PairRows rows;
   for (;;) {
+    // ---- while the scalar warp is on its own: wait for the cell that is being fetched and load the rows the
+    // first quads need (neither depends on the evaluation point), so that the request finds the thread ready
+    pair_wait(pc);
+    if (__double2hiint(creg[PT::NREG - 1]) == 0x7ffdead0) asm volatile("nanosleep.u32 1;");  // = wait for the loads
+    rows.preload(pc.strip_s);
     pbar_sync(bar0 + PB_REQ);
     const int rq = reqbuf[0];
     if (rq & REQ_QUIT) {  // pair-uniform
@@ -211,10 +224,7 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
     const int kind = (rq >> 1) & 7;  // pair-uniform
     const int rpar = (rq >> 6) & 1;
     const double wF = wbuf[0], wS = wbuf[PT::NS];
-    if (active) {
-      pair_wait(pc);
-      pair_contract(creg, pc.strip_s, part_s, wS, wF);
-    }
+    if (active) pair_contract(creg, rows, pc.strip_s, part_s, wS, wF);
     __syncwarp();
     pbar_arrive(bar0 + PB_DONE);
     // ---- the scalar warp has located the point: a wrong cell is redone; then the guessed cell of the next
@@ -227,7 +237,8 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
       if (redo) {
         pair_fetch(table, pc, creg, redo_cell);
         pair_wait(pc);
-        pair_contract(creg, pc.strip_s, part_s, wS, wF);
+        rows.preload(pc.strip_s);
+        pair_contract(creg, rows, pc.strip_s, part_s, wS, wF);
       }
       __syncwarp();
       pbar_arrive(bar0 + PB_D2);
@@ -341,6 +352,7 @@ __device__ __forceinline__ void scalar_round(const TraceConst& tc, unsigned char
     unit_power(tc.saw_m, g.ca, g.sa, cm, sm);
     g.sn = fma(sm, cb, cm * sb);
     g.cs = fma(cm, cb, -sm * sb);
+    eval_wave_terms(tc, g);
   }
 #pragma unroll
   for (int c = 0; c < 4; ++c) S[c] = 0.0;
@@ -410,7 +422,7 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
   }
   double* ks = reinterpret_cast<double*>(smem + PT::OFF_KS) + slot;  // k_j component c at ks[(j*4+c)*NS]
 #pragma unroll 1
-  for (int j = 0; j < 28; ++j) ks[j * NS] = 0.0;
+  for (int j = 0; j < 24; ++j) ks[j * NS] = 0.0;
   double ys[4] = {1.0, 0.0, 0.0, 0.0};  // the state at the start of the step
   double dt = 0.0;                      // the controller's step length
   float base[3] = {0.f, 0.f, 0.f};      // start point of the attempt in cell units (next-cell guess)
@@ -593,8 +605,10 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
         // over the first six derivatives
         scalar_round<MODEL>(tc, smem, slot, bar0, stepping, r, sr, fma(DP_C[r], h, t), X, mu, ratio, base, pos, dy, B_,
                             level, PAIR_SUMS[r], ks, S);
+        if (r < 5) {  // k_7 stays in registers: it is the next step's k_1 (or nothing)
 #pragma unroll
-        for (int c = 0; c < 4; ++c) ks[((r + 1) * 4 + c) * NS] = dy[c];
+          for (int c = 0; c < 4; ++c) ks[((r + 1) * 4 + c) * NS] = dy[c];
+        }
       }
       rounds += 6;
       // PAPER.md:85 Eq. 4 with c = (1,1,1,v_total), state and derivative at the start of the step
@@ -615,7 +629,7 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
       if (MODE != MODE_STEP_ONCE && (!(chk == chk) || fabs(chk) > 1.7e308)) {
         // the derivatives of this attempt will meet zero coefficients in the next one's sums: keep them finite
 #pragma unroll 1
-        for (int j = 4; j < 28; ++j) ks[j * NS] = 0.0;
+        for (int j = 4; j < 24; ++j) ks[j * NS] = 0.0;
       }
       bool accepted = false;
       double dtn = h;
@@ -661,7 +675,7 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
 #pragma unroll
           for (int j = 0; j < 7; ++j)
 #pragma unroll
-            for (int c = 0; c < 4; ++c) a.kall[((long long)j * 4 + c) * n + idx] = ks[(j * 4 + c) * NS];
+            for (int c = 0; c < 4; ++c) a.kall[((long long)j * 4 + c) * n + idx] = j < 6 ? ks[(j * 4 + c) * NS] : dy[c];
           active = false;
           report = REPORT_NO_STATUS;
         }

@@ -106,6 +106,12 @@ typedef struct {
   int32_t saw_on;              /* 1: shear Alfven wave, Boozer only              */
   int32_t saw_m, saw_n;        /* Phi = Phi0 exp(-(s-s0)^2/w2) sin(m theta - n zeta + omega t)  */
   double saw_Phi0, saw_s0, saw_w2, saw_omega;
+  int32_t loss_time_mode;      /* loss time tau: 0 = end time of the first accepted step that ends
+                                  beyond the boundary, the end state returned (S5); 1 = root inside that
+                                  step: cubic Hermite interpolant of the stepped variables through the step's end
+                                  states and end derivatives, bisected to the first observed point with s >= 1,
+                                  that point and its time returned (S5b; Boozer only)        */
+  int32_t reserved_;           /* 0                                                              */
 } catapult_trace_params;
 
 /* ---- field tables ------------------------------------------------

@@ -378,6 +378,35 @@ static int orc_is_lost(const orc_field *f, const double y[4]) {
   return psi >= f->psi0;
 }
 
+/* DESIGN.md reading S5b.  The step from (y0, derivative k0) to (y1, derivative k1) of length h crossed the loss
+ * boundary: orc_is_lost(y0) is false, orc_is_lost(y1) true.  The stepped variables are interpolated inside the step
+ * by the cubic Hermite polynomial of the two end states and end derivatives (both are at hand: k1 is the step's
+ * seventh stage, first-same-as-last), theta in [0,1]:
+ *   y(theta) = (2 th^3 - 3 th^2 + 1) y0 + (th^3 - 2 th^2 + th) h k0 + (-2 th^3 + 3 th^2) y1 + (th^3 - th^2) h k1.
+ * The loss time is t + theta* h with theta* found by 48 bisections on "orc_is_lost(y(theta))" from [0,1]: the
+ * smallest theta the bisection observes beyond the boundary; the returned state is y(theta*). */
+void orc_hermite_state(const double y0[4], const double k0[4], const double y1[4], const double k1[4], double h,
+                       double theta, double y[4]) {
+  const double t2 = theta * theta, t3 = t2 * theta;
+  const double h00 = 2.0 * t3 - 3.0 * t2 + 1.0, h10 = t3 - 2.0 * t2 + theta;
+  const double h01 = -2.0 * t3 + 3.0 * t2, h11 = t3 - t2;
+  for (int i = 0; i < 4; ++i) y[i] = h00 * y0[i] + h10 * h * k0[i] + h01 * y1[i] + h11 * h * k1[i];
+}
+
+double orc_loss_refine(const orc_field *f, const double y0[4], const double k0[4], const double y1[4],
+                       const double k1[4], double h, double y[4]) {
+  double lo = 0.0, hi = 1.0;
+  for (int it = 0; it < 48; ++it) {
+    const double mid = 0.5 * (lo + hi);
+    double ym[4];
+    orc_hermite_state(y0, k0, y1, k1, h, mid, ym);
+    if (orc_is_lost(f, ym)) hi = mid;
+    else lo = mid;
+  }
+  orc_hermite_state(y0, k0, y1, k1, h, hi, y);
+  return hi;
+}
+
 typedef struct {
   const orc_field *f;
   const orc_params *p;
@@ -444,6 +473,21 @@ static void orc_trace_one(const orc_field *f, const orc_params *p, const double 
       }
       consecutive = 0;
       ++nacc;
+      if (p->loss_time_mode == 1 && orc_is_lost(f, ynew)) { /* reading S5b: the loss time inside this step */
+        double yl[4];
+        const double theta = orc_loss_refine(f, y, k1, ynew, k7, h, yl);
+        t = t + theta * h;
+        for (int i = 0; i < 4; ++i) y[i] = yl[i];
+        if (traj && nrec < maxrec) {
+          double xs[4];
+          orc_y_to_state(f, y, xs);
+          traj[nrec * 5] = t;
+          for (int i = 0; i < 4; ++i) traj[nrec * 5 + 1 + i] = xs[i];
+          ++nrec;
+        }
+        st = 1;
+        break;
+      }
       t = clamped ? p->T : t + h;
       if (!clamped) dt = dtn; /* the clamp does not shrink the controller's memory */
       for (int i = 0; i < 4; ++i) { y[i] = ynew[i]; k1[i] = k7[i]; }
@@ -516,6 +560,14 @@ int64_t orc_trace_scripted(const orc_field *f, const orc_params *p, const double
     orc_dp5_attempt(orc_rhs_cb, &ctx, 4, t, y, k1, hh, ynew, k7, err, NULL);
     if (r) r[taken] = orc_error_ratio(4, err, y, k1, hh, p->rtol, p->atol, cscale);
     ++taken;
+    if (p->loss_time_mode == 1 && orc_is_lost(f, ynew)) { /* reading S5b */
+      double yl[4];
+      const double theta = orc_loss_refine(f, y, k1, ynew, k7, hh, yl);
+      t = t + theta * hh;
+      for (int i = 0; i < 4; ++i) y[i] = yl[i];
+      st = 1;
+      break;
+    }
     t = t + hh;
     for (int i = 0; i < 4; ++i) { y[i] = ynew[i]; k1[i] = k7[i]; }
     if (orc_is_lost(f, y)) { st = 1; break; }

@@ -80,7 +80,16 @@ typedef struct {
   int32_t max_consecutive_rejects; /* 0 => 500 */
   int32_t saw_on, saw_m, saw_n;
   double saw_Phi0, saw_s0, saw_w2, saw_omega; /* Phi0 exp(-(s-s0)^2/w2) sin(m th - n ze + omega t) */
+  int32_t loss_time_mode;      /* 0: end of the step that crossed (reading S5); 1: root inside it (reading S5b) */
+  int32_t reserved_;
 } orc_params;
+
+/* ---- loss time inside the last step (reading S5b; tau, "the first time the particle
+ * is observed beyond the boundary", sharpened) ---- */
+void orc_hermite_state(const double y0[4], const double k0[4], const double y1[4], const double k1[4], double h,
+                       double theta, double y[4]);
+double orc_loss_refine(const orc_field *f, const double y0[4], const double k0[4], const double y1[4],
+                       const double k1[4], double h, double y[4]);
 
 /* ---- tricubic ---- */
 void orc_lagrange4(double u, double L[4]);

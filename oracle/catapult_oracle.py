@@ -38,6 +38,7 @@ class CParams(C.Structure):
         ("saw_on", C.c_int32), ("saw_m", C.c_int32), ("saw_n", C.c_int32),
         ("saw_Phi0", C.c_double), ("saw_s0", C.c_double), ("saw_w2", C.c_double),
         ("saw_omega", C.c_double),
+        ("loss_time_mode", C.c_int32), ("reserved_", C.c_int32),
     ]
 
 
@@ -56,6 +57,7 @@ def lib():
         L.orc_trace_record.restype = C.c_int64
         L.orc_trace_scripted.restype = C.c_int64
         L.orc_max_threads.restype = C.c_int
+        L.orc_loss_refine.restype = C.c_double
     return _lib
 
 
@@ -280,6 +282,21 @@ def trace_scripted(f: Field, p: CParams, x0, h):
     n = lib().orc_trace_scripted(f.ref, C.byref(p), _dp(x0), C.c_int64(h.size), _dp(h), _dp(xf),
                                  C.byref(ts), C.byref(st), _dp(r))
     return xf, ts.value, st.value, r[:n].copy()
+
+
+def hermite_state(y0, k0, y1, k1, h: float, theta: float) -> np.ndarray:
+    """Cubic Hermite interpolant of a step's end states and end derivatives at theta in [0,1] (reading S5b)."""
+    y = np.zeros(4)
+    lib().orc_hermite_state(_dp(_f64(y0)), _dp(_f64(k0)), _dp(_f64(y1)), _dp(_f64(k1)), C.c_double(h),
+                            C.c_double(theta), _dp(y))
+    return y
+
+
+def loss_refine(f: Field, y0, k0, y1, k1, h: float):
+    """theta* in (0,1] and y(theta*): where the Hermite interpolant of the step crosses the loss boundary."""
+    y = np.zeros(4)
+    th = lib().orc_loss_refine(f.ref, _dp(_f64(y0)), _dp(_f64(k0)), _dp(_f64(y1)), _dp(_f64(k1)), C.c_double(h), _dp(y))
+    return th, y
 
 
 def estimate(g_kind, status=None, tstop=None, g_user=None):

@@ -49,7 +49,8 @@ class TraceParams(C.Structure):
                 ("dt0", C.c_double), ("dtmax", C.c_double), ("max_steps", C.c_int64),
                 ("max_consecutive_rejects", C.c_int32), ("saw_on", C.c_int32),
                 ("saw_m", C.c_int32), ("saw_n", C.c_int32), ("saw_Phi0", C.c_double),
-                ("saw_s0", C.c_double), ("saw_w2", C.c_double), ("saw_omega", C.c_double)]
+                ("saw_s0", C.c_double), ("saw_w2", C.c_double), ("saw_omega", C.c_double),
+                ("loss_time_mode", C.c_int32), ("reserved_", C.c_int32)]
 
 
 class CatapultError(RuntimeError):

@@ -104,6 +104,9 @@ static catapult_status make_trace_const(const catapult_field* f, const catapult_
     return fail(CATAPULT_EINVAL, "rtol/atol must be finite, non-negative, not both zero");
   if (p->max_steps < 0 || p->max_consecutive_rejects < 0)
     return fail(CATAPULT_EINVAL, "max_steps / max_consecutive_rejects must be >= 0");
+  if (p->loss_time_mode != 0 && p->loss_time_mode != 1) return fail(CATAPULT_EINVAL, "loss_time_mode must be 0 or 1");
+  if (p->loss_time_mode == 1 && f->desc.coord != CATAPULT_COORD_BOOZER)
+    return fail(CATAPULT_EUNSUPPORTED, "loss_time_mode 1 (loss time inside the step) is built for Boozer tracing only");
   if (p->saw_on) {
     if (f->desc.coord != CATAPULT_COORD_BOOZER)
       return fail(CATAPULT_EUNSUPPORTED, "the shear Alfven wave is built for Boozer tracing only");
@@ -137,6 +140,7 @@ static catapult_status make_trace_const(const catapult_field* f, const catapult_
   tc->dtmax = dtmax;
   tc->max_steps = p->max_steps;
   tc->max_rej = p->max_consecutive_rejects > 0 ? p->max_consecutive_rejects : 500;
+  tc->loss_time_mode = p->loss_time_mode;
   tc->saw_m = p->saw_m;
   tc->saw_n = p->saw_n;
   tc->saw_Phi0 = p->saw_Phi0;

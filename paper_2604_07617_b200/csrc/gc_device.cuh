@@ -156,6 +156,33 @@ __device__ __forceinline__ void y_to_state(const double y[4], double x[4]) {
   }
 }
 
+// Loss time inside the step that crossed the boundary (include/catapult.h loss_time_mode 1; S5b; Boozer:
+// s = sqrt(y0^2 + y1^2)).  y(theta) is the cubic Hermite interpolant through the step's end states (ya, yb) and end
+// derivatives (ka, kb; kb is the step's seventh stage), theta in [0, 1].  48 bisections from [0, 1] on "s(theta) >= 1":
+// returns the smallest theta observed beyond the boundary and leaves y(theta) in yb.  Once per lost particle.
+__device__ __forceinline__ void hermite_state(const double ya[4], const double ka[4], const double yb[4],
+                                              const double kb[4], double h, double th, double y[4]) {
+  const double t2 = th * th, t3 = t2 * th;
+  const double h00 = 2.0 * t3 - 3.0 * t2 + 1.0, h10 = t3 - 2.0 * t2 + th, h01 = -2.0 * t3 + 3.0 * t2, h11 = t3 - t2;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) y[i] = h00 * ya[i] + h10 * h * ka[i] + h01 * yb[i] + h11 * h * kb[i];
+}
+__device__ __forceinline__ double loss_refine_boozer(const double ya[4], const double ka[4], double yb[4],
+                                                     const double kb[4], double h) {
+  double lo = 0.0, hi = 1.0, ym[4];
+#pragma unroll 1
+  for (int it = 0; it < 48; ++it) {
+    const double mid = 0.5 * (lo + hi);
+    hermite_state(ya, ka, yb, kb, h, mid, ym);
+    if (::sqrt(fma(ym[0], ym[0], ym[1] * ym[1])) >= 1.0) hi = mid;
+    else lo = mid;
+  }
+  hermite_state(ya, ka, yb, kb, h, hi, ym);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) yb[i] = ym[i];
+  return hi;
+}
+
 template <int MODEL>
 __device__ __forceinline__ bool is_lost(const TraceConst& tc, double level) {
   return (MODEL == MODEL_CART) ? (level >= tc.f.psi0) : (level >= 1.0);

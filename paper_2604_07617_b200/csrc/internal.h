@@ -28,6 +28,7 @@ struct TraceConst {
   double T, rtol, atol, dt0, dtmax;  // dt0 / dtmax <= 0: DESIGN.md S3 defaults, resolved on the device
   long long max_steps;
   int max_rej;
+  int loss_time_mode;  // include/catapult.h
   int saw_m, saw_n;
   double saw_Phi0, saw_s0, saw_invw2, saw_omega, saw_inv_omG;
 };

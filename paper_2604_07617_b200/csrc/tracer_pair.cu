@@ -687,7 +687,15 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
           } else {
             consecutive = 0;
             ++nacc;
-            t = clamped ? tc.T : t + h;
+            const bool lost = is_lost<MODEL>(tc, level);
+            if (lost && tc.loss_time_mode == 1) {
+              // DESIGN.md S5b: the loss time and state inside this step (Hermite interpolant, bisection)
+              const double ka[4] = {ks[0], ks[NS], ks[2 * NS], ks[3 * NS]};
+              const double theta = loss_refine_boozer(ys, ka, X, dy, h);  // X <- y(theta)
+              t = __dadd_rn(t, __dmul_rn(theta, h));
+            } else {
+              t = clamped ? tc.T : t + h;
+            }
             if (!clamped) dt = dtn;
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
@@ -695,7 +703,7 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
               ks[c * NS] = dy[c];  // first-same-as-last
             }
             // DESIGN.md S5: loss first, then T
-            if (is_lost<MODEL>(tc, level)) finish = CATAPULT_ST_LOST;
+            if (lost) finish = CATAPULT_ST_LOST;
             else if (MODE != MODE_SCRIPT && t >= tc.T) finish = CATAPULT_ST_REACHED_T;
           }
         }

@@ -709,3 +709,67 @@ def test_device_math_parity(K):
     assert rel(p5, a ** -0.2) <= 8 * eps and rel(p3, a ** (-1.0 / 3.0)) <= 8 * eps
     bad = K.catapult_math_probe(K.FN_POW_NEG_INV, _dev(np.array([np.inf, np.nan, 1e300])))
     assert not torch.any(bad[1] >= 0.2 / 0.9)       # the controller's floor takes over
+
+
+# ---- f3: loss time inside the crossing step (loss_time_mode 1, S5b) ------------------------------
+@pytest.mark.parametrize("idx", [0, 4])
+def test_loss_time_inside_the_step(K, oracle, cases, idx):
+    """include/catapult.h loss_time_mode 1: the loss time and state are the first point of the crossing step's cubic
+    Hermite interpolant that the bisection observes beyond s = 1.  Scripted replay (both sides walk the oracle's
+    accepted step sequence, so that no floating-point decision separates them before the crossing step): stop
+    times to 1e-8 of the step length and states to 1e-8, the trajectory bar (the root inherits the ~1e-12 agreement
+    of the end states divided by the radial speed per step; observed 2e-10).  Adaptive run: mode 1 changes nothing but the stop time and state
+    of lost particles, which end ON the boundary instead of beyond it."""
+    c = cases[idx]
+    cfg = c["cfg"]
+    x0 = cfg["x0"].copy()
+    n = x0.shape[1]
+    x0[0, ::3] = 0.992 + 0.007 * np.linspace(0.0, 1.0, len(x0[0, ::3]))   # born close to the edge: many are lost
+    T = 2e-5
+    p0 = dict(cfg["params"], T=T)
+    p1 = dict(p0, loss_time_mode=1)
+    op0, op1 = oracle.make_params(p0), oracle.make_params(p1)
+    recs = [oracle.trace_record(c["of"], op0, x0[:, i]) for i in range(n)]
+    hs = [np.diff(r[0][:, 0]) for r in recs]
+    H = np.zeros((max(len(h) for h in hs) + 1, n))
+    for i, h in enumerate(hs):
+        H[:len(h), i] = h
+    g = K.catapult_trace_scripted(c["gf"], p1, _dev(x0), _dev(H))
+    gx, gt, gs = (g[k].cpu().numpy() for k in ("xf", "tstop", "status"))
+    sc = _state_scale(cfg["field"]["coord"])
+    nlost, worst, worst_t = 0, 0.0, 0.0
+    for i in range(n):
+        xo, to, so, _ = oracle.trace_scripted(c["of"], op1, x0[:, i], hs[i])
+        assert gs[i] == so
+        if so != 1:
+            assert gt[i] == to
+            continue
+        nlost += 1
+        hlast = hs[i][-1]
+        assert to <= recs[i][1] and to > recs[i][1] - hlast          # inside the crossing step
+        worst_t = max(worst_t, abs(gt[i] - to) / hlast)
+        d = _state_diff(cfg["field"]["coord"], gx[:, i:i + 1], xo[:, None])[:, 0]
+        worst = max(worst, (np.abs(d) / np.maximum(sc, np.abs(xo))).max())
+        assert 1.0 <= gx[0, i] < 1.0 + 1e-9
+    print(f"cfg{idx}: {nlost} lost; loss time inside the step: worst difference {worst_t:.2e} of the step, state {worst:.2e}")
+    assert nlost >= 8
+    assert worst_t <= 1e-8 and worst <= 1e-8
+    # adaptive runs: the mode touches lost particles only
+    g0 = K.catapult_trace(c["gf"], p0, _dev(x0))
+    g1 = K.catapult_trace(c["gf"], p1, _dev(x0))
+    s0, s1 = g0["status"].cpu().numpy(), g1["status"].cpu().numpy()
+    assert np.array_equal(s0, s1) and np.array_equal(g0["nacc"].cpu().numpy(), g1["nacc"].cpu().numpy())
+    kept, lost = s0 == 0, s0 == 1
+    assert np.array_equal(g0["xf"].cpu().numpy()[:, kept], g1["xf"].cpu().numpy()[:, kept])
+    t0, t1 = g0["tstop"].cpu().numpy(), g1["tstop"].cpu().numpy()
+    assert np.all(t1[lost] <= t0[lost]) and np.any(t1[lost] < t0[lost])
+    s_end = g1["xf"].cpu().numpy()[0, lost]
+    assert np.all((s_end >= 1.0) & (s_end < 1.0 + 1e-9))
+
+
+def test_loss_time_mode_is_validated(K, cases):
+    c3, c0 = cases[3], cases[0]
+    with pytest.raises(K.CatapultError):   # cylindrical model: not built
+        K.catapult_trace(c3["gf"], dict(c3["cfg"]["params"], loss_time_mode=1), _dev(c3["cfg"]["x0"]))
+    with pytest.raises(K.CatapultError):
+        K.catapult_trace(c0["gf"], dict(c0["cfg"]["params"], loss_time_mode=2), _dev(c0["cfg"]["x0"]))

@@ -254,3 +254,65 @@ def test_step_sequences_are_not_reproducible_across_arithmetics(oracle):
         assert np.all(np.abs(ya - yb) <= 8 * a["nacc"][None, :] * 1e-9 * scale)
     assert out[0] < 0.5, out      # measured: 5 of 64 particles keep their counts
     assert out[3] == 1.0, out     # measured: 50 of 50
+
+
+def test_hermite_interpolant_reproduces_cubic_motion(oracle):
+    """Reading S5b: the interpolant of a step's end states and end derivatives is exact for motion that is cubic
+    in time (closed form, retyped here), and hits both ends."""
+    O = oracle
+    rng = np.random.default_rng(11)
+    c = rng.normal(size=(4, 4))                    # y_i(t) = c0 + c1 t + c2 t^2 + c3 t^3
+    yt = lambda t: c[:, 0] + c[:, 1] * t + c[:, 2] * t ** 2 + c[:, 3] * t ** 3
+    dyt = lambda t: c[:, 1] + 2 * c[:, 2] * t + 3 * c[:, 3] * t ** 2
+    t0, h = 0.3, 0.7
+    for th in (0.0, 0.125, 0.5, 0.9, 1.0):
+        y = O.hermite_state(yt(t0), dyt(t0), yt(t0 + h), dyt(t0 + h), h, th)
+        assert np.allclose(y, yt(t0 + th * h), rtol=0, atol=1e-14)
+
+
+def test_loss_refine_finds_the_crossing_of_a_known_orbit(oracle):
+    """Reading S5b on an outward spiral in the pseudo-Cartesian plane whose radius s(t) is known in closed form:
+    y = (s cos w t, s sin w t) with s(t) = s0 + v t crosses s = 1 at t* = (1 - s0)/v.  The cubic interpolant of a
+    short step finds t* to O(h^4); the bracket is as tight as 48 bisections make it."""
+    O = oracle
+    cfg = W.config(0, n=1, T=1e-6)
+    f = O.Field(cfg["field"])
+    s0, v, w = 0.98, 40.0, 300.0
+    y = lambda t: np.array([(s0 + v * t) * math.cos(w * t), (s0 + v * t) * math.sin(w * t), 0.1 + t, 1e5])
+    dy = lambda t: np.array([v * math.cos(w * t) - (s0 + v * t) * w * math.sin(w * t),
+                             v * math.sin(w * t) + (s0 + v * t) * w * math.cos(w * t), 1.0, 0.0])
+    tstar = (1.0 - s0) / v
+    errs = []
+    for h in (8e-4, 4e-4):
+        t0 = tstar - 0.37 * h
+        th, yl = O.loss_refine(f, y(t0), dy(t0), y(t0 + h), dy(t0 + h), h)
+        assert 0.0 < th <= 1.0
+        assert math.hypot(yl[0], yl[1]) >= 1.0                      # the returned state is beyond the boundary ...
+        ybelow = O.hermite_state(y(t0), dy(t0), y(t0 + h), dy(t0 + h), h, th - 2.0 ** -40)
+        assert math.hypot(ybelow[0], ybelow[1]) < 1.0               # ... and a hair earlier it is not
+        errs.append(abs(t0 + th * h - tstar))
+    assert errs[0] < 1e-3 * 8e-4                                    # far inside the step
+    assert errs[1] < errs[0] / 8.0                                  # fourth order in h (16x; 8x asserted)
+
+
+def test_loss_time_mode_sharpens_the_loss_time(oracle):
+    """Reading S5 puts the loss time at the END of the crossing step (an error of up to one step length); reading
+    S5b inside it.  Against a run at a 100x tighter tolerance (steps ~2.5x shorter, orbit converged to 1e-9) the
+    refined loss times of a loose run are much closer than the unrefined ones; states that reached T are
+    untouched by the mode; the step counts are identical."""
+    O = oracle
+    cfg = W.config(0, n=64, T=1e-4)
+    f = O.Field(cfg["field"])
+    loose0 = O.trace(f, O.make_params(dict(cfg["params"], rtol=1e-7)), cfg["x0"])
+    loose1 = O.trace(f, O.make_params(dict(cfg["params"], rtol=1e-7, loss_time_mode=1)), cfg["x0"])
+    tight1 = O.trace(f, O.make_params(dict(cfg["params"], rtol=1e-11, loss_time_mode=1)), cfg["x0"])
+    assert np.array_equal(loose0["status"], loose1["status"]) and np.array_equal(loose0["nacc"], loose1["nacc"])
+    kept = loose0["status"] == 0
+    assert np.array_equal(loose0["xf"][:, kept], loose1["xf"][:, kept])
+    lost = np.flatnonzero((loose0["status"] == 1) & (tight1["status"] == 1))
+    assert len(lost) >= 3
+    assert np.all(loose1["tstop"][lost] <= loose0["tstop"][lost])
+    assert np.all(loose1["xf"][0][lost] >= 1.0) and np.all(loose1["xf"][0][lost] < 1.0 + 1e-9)
+    e0 = np.abs(loose0["tstop"][lost] - tight1["tstop"][lost])
+    e1 = np.abs(loose1["tstop"][lost] - tight1["tstop"][lost])
+    assert np.median(e1) < 0.05 * np.median(e0)

@@ -47,7 +47,7 @@ def test_probe_library_exports_its_header():
 def test_struct_layouts_match_header(lib):
     from paper_2604_07617_b200 import binding
     assert C.sizeof(binding.FieldDesc) == 4 * (6 + 16) + 8 * 6 + 8 * 5 + 8 * 3
-    assert C.sizeof(binding.TraceParams) == 8 * 8 + 8 + 4 * 4 + 8 * 4
+    assert C.sizeof(binding.TraceParams) == 8 * 8 + 8 + 4 * 4 + 8 * 4 + 4 * 2   # + loss_time_mode, reserved_
 
 
 def test_argument_validation_without_gpu(lib):

@@ -86,9 +86,13 @@ typedef struct {
   double G0, I0;       /* Boozer covariant components, constants (vacuum: I0 must be 0) */
   double iota0, iota1; /* rotational transform iota(s) = iota0 + iota1*s */
   double psi0;         /* Boozer: toroidal flux/(2pi) at s=1; cyl: psi_edge (loss level) */
-  /* Boozer 1-D profiles on the s-nodes (iota "represented on a regular interpolant grid"):
-     DEVICE pointers to 3*ncell[0]+1 doubles each, NULL = use the scalars / the linear law above.
-     Non-NULL is valid but not built yet (EUNSUPPORTED): every BASELINE config uses the scalars. */
+  /* Non-vacuum Boozer ("vacuum, finite beta, etc."; R1b): 1-D profiles G(s), I(s), iota(s) on
+     the unique s-nodes (iota "represented on a regular interpolant grid"): pointers to 3*ncell[0]+1
+     doubles each -- device pointers for catapult_field_build, host pointers for catapult_field_build_host --
+     all three or none.  NULL = vacuum: the scalars G0 (I0 = 0) and the linear law above.  The field keeps its
+     own copy (the arrays may be freed after the call returns; for device arrays: after the stream has passed the
+     call).  The profiles are interpolated by the tables' own piecewise cubic (value and derivative).  Every
+     BASELINE config is vacuum; the shear Alfven wave is built on the vacuum model only. */
   const double *G_nodes, *I_nodes, *iota_nodes;
 } catapult_field_desc;
 

@@ -29,6 +29,39 @@ void orc_lagrange4(double u, double L[4]) {
   L[3] = (9.0 / 2.0) * t0 * t1 * t2;
 }
 
+/* derivative of the cubic Lagrange basis on {0, 1/3, 2/3, 1} with respect to u */
+void orc_dlagrange4(double u, double dL[4]) {
+  const double t0 = u, t1 = u - 1.0 / 3.0, t2 = u - 2.0 / 3.0, t3 = u - 1.0;
+  dL[0] = -(9.0 / 2.0) * (t2 * t3 + t1 * t3 + t1 * t2);
+  dL[1] = (27.0 / 2.0) * (t2 * t3 + t0 * t3 + t0 * t2);
+  dL[2] = -(27.0 / 2.0) * (t1 * t3 + t0 * t3 + t0 * t1);
+  dL[3] = (9.0 / 2.0) * (t1 * t2 + t0 * t2 + t0 * t1);
+}
+
+/* A profile given on the unique s-nodes (iota "is represented on a regular interpolant grid"):
+   the cell of s as in orc_locate (clamped: the end cells' cubics are extrapolated), value and
+   derivative with respect to s of that cell's cubic through its four nodes. */
+void orc_profile(const orc_field *f, const double *nodes, double s, double *val, double *dval_ds) {
+  const int k = f->ncell[0];
+  const double h = (f->hi[0] - f->lo[0]) / (double)k;
+  const double t = (s - f->lo[0]) / h;
+  double fi = floor(t);
+  if (fi < 0.0) fi = 0.0;
+  if (fi > (double)(k - 1)) fi = (double)(k - 1);
+  const double u = t - fi;
+  double L[4], dL[4];
+  orc_lagrange4(u, L);
+  orc_dlagrange4(u, dL);
+  const double *F = nodes + 3 * (int64_t)fi;
+  double v = 0.0, d = 0.0;
+  for (int a = 0; a < 4; ++a) {
+    v += L[a] * F[a];
+    d += dL[a] * F[a];
+  }
+  *val = v;
+  *dval_ds = d / h;
+}
+
 static int orc_is_periodic(const orc_field *f, int d) {
   if (f->coord == ORC_COORD_BOOZER) return d >= 1; /* theta, zeta */
   return d == 2;                                   /* phi */
@@ -127,6 +160,29 @@ void orc_gc_boozer(const orc_field *f, const orc_params *p, double mu, double t,
   const double iota = f->iota0 + f->iota1 * s;
   const double W = (M / q) * (vpar * vpar / B + mu);
   const double B_psi = B_s / psi0;
+  if (f->G_nodes) {
+    /* R1b (non-vacuum Boozer, no wave): Euler-Lagrange equations of Eq. 3 with B = G(psi) grad(zeta) +
+       I(psi) grad(theta), A = psi grad(theta) - psi_p grad(zeta), dpsi_p/dpsi = iota; ' = d/dpsi:
+         D = G + iota I + rho (G I' - I G'),  rho = M vpar / (q B)
+         psidot = -W (G B_th - I B_ze) / D
+         thdot  = (G W B_psi + (iota - rho G') vpar B) / D
+         zedot  = ((1 + rho I') vpar B - I W B_psi) / D
+         vdot   = -mu B ((iota - rho G') B_th + (1 + rho I') B_ze) / D                                  */
+    double Gs, dG, Is, dI, io, dio;
+    orc_profile(f, f->G_nodes, s, &Gs, &dG);
+    orc_profile(f, f->I_nodes, s, &Is, &dI);
+    orc_profile(f, f->iota_nodes, s, &io, &dio);
+    const double Gp = dG / psi0, Ip = dI / psi0;
+    const double rho = M * vpar / (q * B);
+    const double D = Gs + io * Is + rho * (Gs * Ip - Is * Gp);
+    const double a = io - rho * Gp, b = 1.0 + rho * Ip;
+    out[0] = -W * (Gs * B_th - Is * B_ze) / D / psi0;
+    out[1] = (Gs * W * B_psi + a * vpar * B) / D;
+    out[2] = (b * vpar * B - Is * W * B_psi) / D;
+    out[3] = -mu * B * (a * B_th + b * B_ze) / D;
+    if (p->saw_on) out[0] = out[1] = out[2] = out[3] = NAN; /* the wave is defined on the vacuum model only */
+    return;
+  }
   if (!p->saw_on) {
     /* R1 (Boozer vacuum) */
     out[0] = -B_th * W / psi0;
@@ -333,7 +389,7 @@ void orc_default_steps(const orc_field *f, const orc_params *p, double *dt0, dou
   double L;
   if (f->coord == ORC_COORD_BOOZER) {
     const double Bref = f->nodes ? fabs(f->nodes[0]) : 1.0;
-    L = fabs(f->G0) / Bref;
+    L = fabs(f->G_nodes ? f->G_nodes[0] : f->G0) / Bref; /* non-vacuum: G on the axis */
   } else {
     L = f->hi[0];
   }

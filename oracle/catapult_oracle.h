@@ -70,6 +70,9 @@ typedef struct {
   double psi0;         /* Boozer: toroidal flux/2pi at s=1; cyl: psi_edge      */
   orc_analytic_fn analytic; /* NULL => tables */
   void *analytic_ctx;
+  /* non-vacuum Boozer ("vacuum, finite beta, etc."; reading R1b): G(s), I(s), iota(s) on the
+     3*ncell[0]+1 unique s-nodes of the grid (all three or none; NULL => the scalars G0, I0 = 0 and the linear law) */
+  const double *G_nodes, *I_nodes, *iota_nodes;
 } orc_field;
 
 typedef struct {
@@ -90,6 +93,10 @@ void orc_hermite_state(const double y0[4], const double k0[4], const double y1[4
                        double theta, double y[4]);
 double orc_loss_refine(const orc_field *f, const double y0[4], const double k0[4], const double y1[4],
                        const double k1[4], double h, double y[4]);
+
+/* ---- 1-D profiles on the s-nodes: value and d/ds by the same piecewise cubic as the tables ---- */
+void orc_dlagrange4(double u, double dL[4]);
+void orc_profile(const orc_field *f, const double *nodes, double s, double *val, double *dval_ds);
 
 /* ---- tricubic ---- */
 void orc_lagrange4(double u, double L[4]);

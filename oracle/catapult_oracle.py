@@ -26,6 +26,7 @@ class CField(C.Structure):
         ("G0", C.c_double), ("I0", C.c_double), ("iota0", C.c_double), ("iota1", C.c_double),
         ("psi0", C.c_double),
         ("analytic", ANALYTIC_FN), ("analytic_ctx", C.c_void_p),
+        ("G_nodes", _c_double_p), ("I_nodes", _c_double_p), ("iota_nodes", _c_double_p),
     ]
 
 
@@ -90,6 +91,12 @@ class Field:
             self.c.nodes = _dp(self.nodes)
         for k in ("G0", "I0", "iota0", "iota1", "psi0"):
             setattr(self.c, k, float(fd.get(k, 0.0)))
+        self.profiles = {}
+        for k in ("G_nodes", "I_nodes", "iota_nodes"):   # non-vacuum Boozer: profiles on the unique s-nodes
+            if fd.get(k) is not None:
+                self.profiles[k] = _f64(fd[k])
+                assert self.profiles[k].shape == (3 * int(fd["ncell"][0]) + 1,), self.profiles[k].shape
+                setattr(self.c, k, _dp(self.profiles[k]))
         self._cb = None
         if analytic is not None:
             m = self.c.nquant
@@ -282,6 +289,14 @@ def trace_scripted(f: Field, p: CParams, x0, h):
     n = lib().orc_trace_scripted(f.ref, C.byref(p), _dp(x0), C.c_int64(h.size), _dp(h), _dp(xf),
                                  C.byref(ts), C.byref(st), _dp(r))
     return xf, ts.value, st.value, r[:n].copy()
+
+
+def profile(f: Field, nodes, s: float):
+    """value and d/ds of a profile tabulated on the unique s-nodes (the tables' piecewise cubic)"""
+    v, d = C.c_double(0), C.c_double(0)
+    nodes = _f64(nodes)
+    lib().orc_profile(f.ref, _dp(nodes), C.c_double(s), C.byref(v), C.byref(d))
+    return v.value, d.value
 
 
 def hermite_state(y0, k0, y1, k1, h: float, theta: float) -> np.ndarray:

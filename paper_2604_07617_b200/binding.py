@@ -140,9 +140,19 @@ def make_desc(fd: dict) -> FieldDesc:
         setattr(d, k, float(fd.get(k, 0.0)))
     for i, tag in enumerate(fd.get("quant", ())):
         d.quant[i] = int(tag)
-    for k in ("G_nodes", "I_nodes", "iota_nodes"):        # device pointers (CUDA tensors) or absent
+    keep = []
+    for k in ("G_nodes", "I_nodes", "iota_nodes"):        # CUDA tensors (device pointers), numpy arrays, or absent
         t = fd.get(k)
-        setattr(d, k, None if t is None else t.data_ptr())
+        if t is None:
+            setattr(d, k, None)
+        elif isinstance(t, np.ndarray):                    # host array: the library copies it (any direction)
+            t = np.ascontiguousarray(t, dtype=np.float64)
+            keep.append(t)
+            setattr(d, k, t.ctypes.data)
+        else:
+            keep.append(t)
+            setattr(d, k, t.data_ptr())
+    d._keep = keep                                         # alive until the build call has returned
     return d
 
 

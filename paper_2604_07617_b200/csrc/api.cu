@@ -58,13 +58,17 @@ static catapult_status validate_desc(const catapult_field_desc* d) {
   }
   if (d->nfp < 1) return fail(CATAPULT_EINVAL, "desc.nfp must be >= 1");
   if (d->coord == CATAPULT_COORD_BOOZER) {
-    if (d->G_nodes || d->I_nodes || d->iota_nodes)
-      return fail(CATAPULT_EUNSUPPORTED, "tabulated G(s) / I(s) / iota(s) profiles are not built (use the scalars)");
-    if (d->I0 != 0.0) return fail(CATAPULT_EUNSUPPORTED, "non-vacuum Boozer (I0 != 0) is not built");
+    const int nprof = (d->G_nodes != nullptr) + (d->I_nodes != nullptr) + (d->iota_nodes != nullptr);
+    if (nprof != 0 && nprof != 3)
+      return fail(CATAPULT_EINVAL, "G_nodes, I_nodes and iota_nodes: give all three (non-vacuum Boozer) or none");
+    if (nprof == 0 && d->I0 != 0.0)
+      return fail(CATAPULT_EUNSUPPORTED, "non-vacuum Boozer is built with tabulated profiles: give G_nodes, I_nodes, iota_nodes");
     if (!(std::isfinite(d->G0) && d->G0 != 0.0)) return fail(CATAPULT_EINVAL, "desc.G0 must be finite, non-zero");
     if (!(std::isfinite(d->psi0) && d->psi0 != 0.0)) return fail(CATAPULT_EINVAL, "desc.psi0 must be finite, non-zero");
-  } else if (!std::isfinite(d->psi0)) {
-    return fail(CATAPULT_EINVAL, "desc.psi0 (psi_edge) must be finite");
+  } else {
+    if (d->G_nodes || d->I_nodes || d->iota_nodes)
+      return fail(CATAPULT_EINVAL, "profiles on the s-nodes belong to Boozer tracing");
+    if (!std::isfinite(d->psi0)) return fail(CATAPULT_EINVAL, "desc.psi0 (psi_edge) must be finite");
   }
   return CATAPULT_OK;
 }
@@ -73,6 +77,7 @@ static void fill_field_const(const catapult_field_desc& d, const double* table, 
                              FieldConst* fc) {
   fc->table = table;
   fc->node0 = node0;
+  fc->prof = d.G_nodes ? node0 + 1 : nullptr;  // the field's own copy of the three profiles sits behind node0
   fc->coord = d.coord;
   fc->m = d.nquant;
   for (int i = 0; i < 3; ++i) {
@@ -148,7 +153,11 @@ static catapult_status make_trace_const(const catapult_field* f, const catapult_
   tc->saw_invw2 = p->saw_on ? 1.0 / p->saw_w2 : 0.0;
   tc->saw_omega = p->saw_omega;
   tc->saw_inv_omG = p->saw_on ? f->fc.invG / p->saw_omega : 0.0;
-  *model = f->desc.coord == CATAPULT_COORD_CYL ? MODEL_CART : (p->saw_on ? MODEL_BOOZER_SAW : MODEL_BOOZER_VAC);
+  if (f->fc.prof && p->saw_on)
+    return fail(CATAPULT_EUNSUPPORTED, "the shear Alfven wave is built on the vacuum Boozer model only");
+  *model = f->desc.coord == CATAPULT_COORD_CYL
+               ? MODEL_CART
+               : (f->fc.prof ? MODEL_BOOZER_NV : (p->saw_on ? MODEL_BOOZER_SAW : MODEL_BOOZER_VAC));
   return CATAPULT_OK;
 }
 
@@ -192,7 +201,9 @@ catapult_status catapult_field_build(const catapult_field_desc* desc, const doub
   f->built = nullptr;
   // stream-ordered allocation: the build neither blocks the host nor synchronises the device
   cudaError_t e = cudaGetDevice(&f->device);
-  if (e == cudaSuccess) e = cudaMallocAsync((void**)&f->d_table, f->table_bytes + sizeof(double), (cudaStream_t)stream);
+  const size_t nprof = desc->G_nodes ? (size_t)(3 * desc->ncell[0] + 1) : 0;  // non-vacuum Boozer: three profiles
+  if (e == cudaSuccess)
+    e = cudaMallocAsync((void**)&f->d_table, f->table_bytes + (1 + 3 * nprof) * sizeof(double), (cudaStream_t)stream);
   if (e != cudaSuccess) {
     delete f;
     return cuda_fail(e, "cudaMallocAsync(table)");
@@ -200,6 +211,14 @@ catapult_status catapult_field_build(const catapult_field_desc* desc, const doub
   double* d_node0 = f->d_table + f->table_bytes / sizeof(double);
   fill_field_const(*desc, f->d_table, d_node0, &f->fc);
   st = launch_field_build(*desc, d_nodes, f->d_table, d_node0, (cudaStream_t)stream);
+  if (st == CATAPULT_OK && nprof) {  // the field keeps its own copy: the caller's arrays may go after this call
+    const double* src[3] = {desc->G_nodes, desc->I_nodes, desc->iota_nodes};
+    for (int k = 0; k < 3 && e == cudaSuccess; ++k)
+      e = cudaMemcpyAsync(d_node0 + 1 + k * nprof, src[k], nprof * sizeof(double), cudaMemcpyDefault,
+                          (cudaStream_t)stream);
+    if (e != cudaSuccess) st = cuda_fail(e, "cudaMemcpyAsync(profiles)");
+    f->desc.G_nodes = f->desc.I_nodes = f->desc.iota_nodes = d_node0 + 1;  // marks "non-vacuum"; not the caller's
+  }
   if (st == CATAPULT_OK) {
     e = cudaEventCreateWithFlags(&f->built, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventRecord(f->built, (cudaStream_t)stream);

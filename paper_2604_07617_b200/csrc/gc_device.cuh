@@ -25,6 +25,7 @@ namespace catapult {
 constexpr int MODEL_BOOZER_VAC = 0;  // DESIGN.md R1
 constexpr int MODEL_BOOZER_SAW = 1;  // DESIGN.md R2
 constexpr int MODEL_CART = 2;        // DESIGN.md R3
+constexpr int MODEL_BOOZER_NV = 3;   // DESIGN.md R1b: non-vacuum Boozer, G(s), I(s), iota(s) tabulated
 
 // ---- cell locate (nearest cell, cubic extrapolated outside) ---------------------
 // reduces x-lo into [0, span) (periodic dimension).  span * floor(.) is exact inside the fma, so the result
@@ -114,6 +115,28 @@ __device__ __forceinline__ double horner64(Get4 get4, double wL, double wS, doub
 #pragma unroll
   for (int a = 0; a < 4; ++a) P[a] = horner_plane(get4, a, wS, wF);
   return horner_row(P[0], P[1], P[2], P[3], wL);
+}
+
+// A profile tabulated on the unique s-nodes (R1b): value and derivative with respect to s of the cubic
+// through the four nodes of the s-cell (the tables' own piecewise-cubic interpolation; end cells extrapolate).
+// u in cell units, invh = cells per unit of s.
+__device__ __forceinline__ void profile_weights(double u, double invh, double L[4], double dL[4]) {
+  const double t0 = u, t1 = u - 1.0 / 3.0, t2 = u - 2.0 / 3.0, t3 = u - 1.0;
+  L[0] = -4.5 * t1 * t2 * t3;
+  L[1] = 13.5 * t0 * t2 * t3;
+  L[2] = -13.5 * t0 * t1 * t3;
+  L[3] = 4.5 * t0 * t1 * t2;
+  dL[0] = -4.5 * invh * (t2 * t3 + t1 * t3 + t1 * t2);
+  dL[1] = 13.5 * invh * (t2 * t3 + t0 * t3 + t0 * t2);
+  dL[2] = -13.5 * invh * (t1 * t3 + t0 * t3 + t0 * t1);
+  dL[3] = 4.5 * invh * (t1 * t2 + t0 * t2 + t0 * t1);
+}
+__device__ __forceinline__ void profile_eval(const double* __restrict__ nodes, int cell, const double L[4],
+                                             const double dL[4], double& v, double& dv) {
+  const double* F = nodes + 3 * cell;
+  const double f0 = __ldg(F), f1 = __ldg(F + 1), f2 = __ldg(F + 2), f3 = __ldg(F + 3);
+  v = fma(L[3], f3, fma(L[2], f2, fma(L[1], f1, L[0] * f0)));
+  dv = fma(dL[3], f3, fma(dL[2], f2, fma(dL[1], f1, dL[0] * f0)));
 }
 
 // Boost odeint default step adjuster for dopri5 (S2):

@@ -16,6 +16,7 @@ namespace catapult {
 struct FieldConst {
   const double* table;  // [cell][quantity][64], cell-major (include/catapult.h)
   const double* node0;  // device scalar: first node of column 0 (written by field_build_kernel)
+  const double* prof;   // non-vacuum Boozer: [3][3 k0 + 1] = G, I, iota on the unique s-nodes; nullptr: scalars
   int coord, m;
   int k[3];
   double lo[3], invh[3], span[3], invspan[3];

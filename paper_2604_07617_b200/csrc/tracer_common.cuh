@@ -130,7 +130,24 @@ struct EvalGeo {
   double sn, cs, Phihat, dPhihat;  // wave terms (MODEL_BOOZER_SAW)
   // ... and what the right-hand side makes of them without the field values (eval_wave_terms)
   double Phi_psi, Phi_th, al_th, iag, iagG, t2;
+  // non-vacuum Boozer (MODEL_BOOZER_NV): G, dG/dpsi, I, dI/dpsi, iota at s (eval_profiles)
+  double Gs, Gp, Is, Ip, io;
 };
+
+// The profiles of R1b at s (R1b): needs only s, so it runs while the contraction does.
+__device__ __forceinline__ void eval_profiles(const FieldConst& f, EvalGeo& g) {
+  const double t = (g.a - f.lo[0]) * f.invh[0];
+  int i = __double2int_rd(t);
+  i = min(max(i, 0), f.k[0] - 1);
+  double L[4], dL[4], dG, dI, dio;
+  profile_weights(t - (double)i, f.invh[0], L, dL);
+  const int np = 3 * f.k[0] + 1;
+  profile_eval(f.prof, i, L, dL, g.Gs, dG);
+  profile_eval(f.prof + np, i, L, dL, g.Is, dI);
+  profile_eval(f.prof + 2 * np, i, L, dL, g.io, dio);
+  g.Gp = dG * f.invpsi0;
+  g.Ip = dI * f.invpsi0;
+}
 
 // The part of R2 that does not need the interpolated field: computed while the
 // contraction is still running.  Same operations, same order as if written inside eval_physics.
@@ -186,6 +203,25 @@ __device__ __forceinline__ void eval_physics(const TraceConst& tc, const double 
     const double B_psi = B_s * f.invpsi0;
     const double vBG = vpar * B * f.invG;
     double sdot, thdot, vdot;
+    if (MODEL == MODEL_BOOZER_NV) {
+      // R1b: D = G + iota I + rho (G I' - I G'), rho = M vpar / (q B), ' = d/dpsi
+      const double rho = tc.Moq * vpar * invB;
+      const double D = fma(rho, fma(g.Gs, g.Ip, -g.Is * g.Gp), fma(g.io, g.Is, g.Gs));
+      const double invD = fm::rcp(D);
+      const double ca = fma(-rho, g.Gp, g.io), cb = fma(rho, g.Ip, 1.0);
+      const double vB = vpar * B;
+      sdot = -W * fma(g.Gs, B_th, -g.Is * B_ze) * invD * f.invpsi0;
+      thdot = fma(g.Gs * W, B_psi, ca * vB) * invD;
+      const double zedot = fma(cb, vB, -g.Is * W * B_psi) * invD;
+      vdot = -mu * B * fma(ca, B_th, cb * B_ze) * invD;
+      dy[0] = fma(sdot, g.ca, -thdot * y[1]);
+      dy[1] = fma(sdot, g.sa, thdot * y[0]);
+      dy[2] = zedot;
+      dy[3] = vdot;
+      modB = B;
+      level = s;
+      return;
+    }
     if (MODEL == MODEL_BOOZER_VAC) {
       sdot = -B_th * W * f.invpsi0;
       thdot = fma(B_psi, W, iota * vBG);

@@ -341,6 +341,7 @@ __device__ __forceinline__ void scalar_round(const TraceConst& tc, unsigned char
   // ---- in the shadow of the contraction: unit vector, wave terms, stage sums
   g.ca = !(g.a > 0.0) ? 1.0 : X[0] * g.inva;
   g.sa = X[1] * g.inva;
+  if (MODEL == MODEL_BOOZER_NV) eval_profiles(f, g);
   if (MODEL == MODEL_BOOZER_SAW) {
     const double ds = g.a - tc.saw_s0;
     g.Phihat = tc.saw_Phi0 * fm::exp(-ds * ds * tc.saw_invw2);
@@ -415,7 +416,8 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
   // DESIGN.md S3: default step lengths (L = |G| / |B|(node 0), read from the device scalar the field build left)
   double dtmax = tc.dtmax, dt0 = tc.dt0;
   if (!(dtmax > 0.0)) {
-    const double L = __ddiv_rn(fabs(tc.f.G), fabs(*tc.f.node0));
+    const double Gaxis = (MODEL == MODEL_BOOZER_NV) ? tc.f.prof[0] : tc.f.G;  // non-vacuum: G on the axis
+    const double L = __ddiv_rn(fabs(Gaxis), fabs(*tc.f.node0));
     dtmax = __ddiv_rn(__dmul_rn(0.5 * 3.14159265358979323846, L), tc.vtot);
     dt0 = dt0 > 0.0 ? dt0 : __dmul_rn(1e-3, dtmax);
     dt0 = dt0 > dtmax ? dtmax : dt0;
@@ -782,6 +784,7 @@ template <int MODE>
 static catapult_status pair_dispatch(const TraceConst& tc, const TraceArgs& a, int model, cudaStream_t s) {
   if (a.n == 0) return CATAPULT_OK;
   if (model == MODEL_BOOZER_VAC) return pair_launch<MODEL_BOOZER_VAC, MODE>(tc, a, s);
+  if (model == MODEL_BOOZER_NV) return pair_launch<MODEL_BOOZER_NV, MODE>(tc, a, s);
   return pair_launch<MODEL_BOOZER_SAW, MODE>(tc, a, s);
 }
 
@@ -796,6 +799,7 @@ catapult_status launch_trace_pair(const TraceConst& tc, const TraceArgs& a, int 
 catapult_status trace_pair_shape(int model, int64_t n, int* blocks, int* threads) {
   int cap = 0;
   if (model == MODEL_BOOZER_VAC) return pair_shape<MODEL_BOOZER_VAC, MODE_ADAPTIVE>(n, blocks, threads, &cap);
+  if (model == MODEL_BOOZER_NV) return pair_shape<MODEL_BOOZER_NV, MODE_ADAPTIVE>(n, blocks, threads, &cap);
   return pair_shape<MODEL_BOOZER_SAW, MODE_ADAPTIVE>(n, blocks, threads, &cap);
 }
 

@@ -239,3 +239,12 @@ def config(idx: int, n: int | None = None, T: float | None = None, ncell=None,
         raise ValueError(f"no config {idx}")
     return dict(name=CONFIG_NAMES[idx], field=field, params=params,
                 x0=np.ascontiguousarray(x0), g_kind=0)
+
+
+def nonvacuum_profiles(ncell0: int) -> dict:
+    """Profiles of a non-vacuum Boozer equilibrium on the 3*ncell0+1 unique s-nodes (a NEXT-row input,
+    not one of BASELINE.json's configs): G(s) = G0 (1 + 0.05 s - 0.02 s^2), I(s) = G0 (0.02 s + 0.01 s^3),
+    iota(s) = 0.42 + 0.1 s + 0.05 s^2.  Merge into a Boozer field dict."""
+    s = np.linspace(0.0, 1.0, 3 * ncell0 + 1)
+    return dict(G_nodes=G0 * (1.0 + 0.05 * s - 0.02 * s ** 2), I_nodes=G0 * (0.02 * s + 0.01 * s ** 3),
+                iota_nodes=0.42 + 0.1 * s + 0.05 * s ** 2)

@@ -773,3 +773,94 @@ def test_loss_time_mode_is_validated(K, cases):
         K.catapult_trace(c3["gf"], dict(c3["cfg"]["params"], loss_time_mode=1), _dev(c3["cfg"]["x0"]))
     with pytest.raises(K.CatapultError):
         K.catapult_trace(c0["gf"], dict(c0["cfg"]["params"], loss_time_mode=2), _dev(c0["cfg"]["x0"]))
+
+
+# ---- f2: non-vacuum Boozer with tabulated profiles (R1b) ----------------------------------------------
+@pytest.fixture(scope="module")
+def nonvacuum_case(K, oracle):
+    cfg = W.config(2, n=45, T=1e-5, ncell=[12, 10, 9])      # config-2 recipe (ragged grid) + G(s), I(s), iota(s)
+    fd = dict(cfg["field"], **W.nonvacuum_profiles(12))
+    return dict(cfg=cfg, fd=fd, gf=K.catapult_field_build(fd), of=oracle.Field(fd), op=oracle.make_params(cfg["params"]))
+
+
+def test_nonvacuum_single_step_parity(K, oracle, nonvacuum_case):
+    """One attempted step from identical state with the non-vacuum right-hand side (R1b): all seven derivatives and the
+    new state to 1e-11, the error ratio to 1e-4 (the bars of test_single_step_parity); and the profiles matter: the
+    vacuum field of the same tables gives different derivatives."""
+    c = nonvacuum_case
+    cfg = c["cfg"]
+    x0 = cfg["x0"].copy()
+    n = x0.shape[1]
+    x0[0, 1::8] = 1e-3                     # near the axis and in the last s-cell too
+    x0[0, 2::8] = 0.97
+    rng = np.random.default_rng(77)
+    t = 1e-6 * rng.random(n)
+    h = cfg["params"]["dtmax"] * (0.02 + 0.1 * rng.random(n))
+    xg, rg, kg = (a.cpu().numpy() for a in K.catapult_step_once(c["gf"], cfg["params"], _dev(x0), _dev(t), _dev(h)))
+    sc = _state_scale(0)
+    worst = worst_k = worst_r = 0.0
+    for i in range(n):
+        xo, ro, ko = oracle.step_once(c["of"], c["op"], x0[:, i], t[i], h[i])
+        d = _stepped(0, xg[:, i]) - _stepped(0, xo)
+        worst = max(worst, (np.abs(d) / sc).max())
+        worst_k = max(worst_k, (np.abs(kg[:, :, i] - ko) / (np.abs(ko).max(axis=0)[None, :] + 1e-300)).max())
+        worst_r = max(worst_r, abs(rg[i] - ro) / max(ro, 1e-3))
+    print(f"non-vacuum single step: state {worst:.2e}, derivatives {worst_k:.2e}, error ratio {worst_r:.2e}")
+    assert worst <= 1e-11 and worst_k <= 1e-11 and worst_r <= 1e-4
+    gv = K.catapult_field_build(cfg["field"])
+    kv = K.catapult_step_once(gv, cfg["params"], _dev(x0), _dev(t), _dev(h))[2].cpu().numpy()
+    assert np.abs(kv[0] - kg[0]).max() > 1e-3 * np.abs(kg[0]).max()
+
+
+def test_nonvacuum_trajectory_parity(K, oracle, nonvacuum_case):
+    """Whole trajectories over 1e-5 s by scripted replay (the bar of test_trajectory_parity_1e5_window: 1e-8), and the
+    free-running adaptive kernel: statuses and accepted-step totals against the adaptive oracle."""
+    c = nonvacuum_case
+    cfg = c["cfg"]
+    x0 = cfg["x0"]
+    n = x0.shape[1]
+    recs = [oracle.trace_record(c["of"], c["op"], x0[:, i]) for i in range(n)]
+    hs = [np.diff(r[0][:, 0]) for r in recs]
+    H = np.zeros((max(len(h) for h in hs) + 1, n))
+    for i, h in enumerate(hs):
+        H[:len(h), i] = h
+    g = K.catapult_trace_scripted(c["gf"], cfg["params"], _dev(x0), _dev(H))
+    gx, gt, gs = (g[k].cpu().numpy() for k in ("xf", "tstop", "status"))
+    sc = _state_scale(0)
+    worst = 0.0
+    for i in range(n):
+        xo, to, so, _ = oracle.trace_scripted(c["of"], c["op"], x0[:, i], hs[i])
+        assert gs[i] == so and gt[i] == to
+        d = _state_diff(0, gx[:, i:i + 1], xo[:, None])[:, 0]
+        worst = max(worst, (np.abs(d) / np.maximum(sc, np.abs(xo))).max())
+    print(f"non-vacuum scripted 1e-5 s window: worst relative difference {worst:.2e}")
+    assert worst <= 1e-8
+    ga = K.catapult_trace(c["gf"], cfg["params"], _dev(x0))
+    oa = oracle.trace(c["of"], c["op"], x0)
+    assert np.array_equal(ga["status"].cpu().numpy(), oa["status"])
+    na = ga["nacc"].cpu().numpy().astype(np.int64)
+    assert abs(na.sum() - oa["nacc"].sum()) <= 0.02 * oa["nacc"].sum()
+
+
+def test_nonvacuum_default_step_lengths(K, oracle, nonvacuum_case):
+    """Reading S3 with profiles: L = |G(s = 0)| / |B|(node 0), resolved on the device from the field's own copy of the
+    profile; bit-exact against orc_default_steps."""
+    c = nonvacuum_case
+    pd = dict(c["cfg"]["params"], dt0=0.0, dtmax=0.0)
+    dt0_o, dtmax_o = oracle.default_steps(c["of"], oracle.make_params(pd))
+    st = K.catapult_trace_init(c["gf"], pd, _dev(c["cfg"]["x0"]).clone())
+    assert torch.all(st["dt"] == dt0_o), (st["dt"][0].item(), dt0_o)
+    st2 = K.catapult_trace_init(c["gf"], dict(pd, dt0=1.0), _dev(c["cfg"]["x0"]).clone())
+    assert torch.all(st2["dt"] == dtmax_o), (st2["dt"][0].item(), dtmax_o)
+
+
+def test_nonvacuum_input_is_validated(K, nonvacuum_case):
+    c = nonvacuum_case
+    with pytest.raises(K.CatapultError):    # all three profiles or none
+        K.catapult_field_build(dict(c["cfg"]["field"], G_nodes=c["fd"]["G_nodes"]))
+    with pytest.raises(K.CatapultError):    # the wave is built on the vacuum model only
+        K.catapult_trace(c["gf"], dict(c["cfg"]["params"], saw_on=1, saw_m=1, saw_n=1, saw_Phi0=1e3, saw_s0=0.5,
+                                       saw_w2=0.01, saw_omega=2 * math.pi * 1e5), _dev(c["cfg"]["x0"]))
+    c3 = W.config(3, n=4, T=1e-6, ncell=[4, 4, 4])
+    with pytest.raises(K.CatapultError):    # profiles belong to Boozer tracing
+        K.catapult_field_build(dict(c3["field"], **W.nonvacuum_profiles(4)))

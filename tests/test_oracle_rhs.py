@@ -225,3 +225,113 @@ def test_cartesian_pphi_and_energy_conserved_axisymmetric(oracle):
         assert np.max(np.abs(E / E[0] - 1)) < 1e-8
         P = M * R * vals[:, 1] / modB * traj[:, 4] + Q * vals[:, 6]
         assert np.max(np.abs(P - P[0])) < 1e-8 * Q * W.PSI_EDGE_CYL
+
+
+# ---- R1b: non-vacuum Boozer with tabulated profiles ("vacuum, finite beta, etc.") ----
+_NV_G = lambda s: W.G0 * (1.0 + 0.05 * s - 0.02 * s ** 2)            # cubic or lower: reproduced exactly by one cell
+_NV_I = lambda s: W.G0 * (0.02 * s + 0.01 * s ** 3)
+_NV_IOTA = lambda s: 0.42 + 0.1 * s + 0.05 * s ** 2
+
+
+def _nonvacuum_fd(ncell0=1):
+    fd = _boozer_fd()
+    fd["ncell"] = [ncell0, 1, 1]
+    sn = np.linspace(0.0, 1.0, 3 * ncell0 + 1)
+    fd.update(G_nodes=_NV_G(sn), I_nodes=_NV_I(sn), iota_nodes=_NV_IOTA(sn))
+    return fd
+
+
+def test_profiles_reproduce_cubics_and_their_derivatives(oracle):
+    """A profile on the unique s-nodes is interpolated by the tables' piecewise cubic: cubics and their derivatives
+    are reproduced to round-off, in the end cells also outside [0, 1] (extrapolation)."""
+    O = oracle
+    for k0 in (1, 3):
+        f = O.Field(_nonvacuum_fd(k0))
+        sn = np.linspace(0.0, 1.0, 3 * k0 + 1)
+        for s in (-0.05, 0.0, 0.2, 1.0 / 3.0, 0.77, 1.0, 1.03):
+            v, d = O.profile(f, _NV_I(sn), s)
+            assert abs(v - _NV_I(s)) <= 1e-13 * W.G0
+            assert abs(d - W.G0 * (0.02 + 0.03 * s ** 2)) <= 1e-12 * W.G0
+
+
+def test_nonvacuum_rhs_equals_euler_lagrange_of_eq3(oracle):
+    """R1b against the Euler-Lagrange equations of Eq. 3 with B = G(psi) grad(zeta) + I(psi) grad(theta),
+    derived here with sympy: L = q (psi + rho I) thdot + q (rho G - psi_p) zedot - H, rho = M v / (q B)."""
+    O = oracle
+    psi, th, ze, v = sp.symbols("psi theta zeta v", real=True)
+    mu = sp.Symbol("mu", positive=True)
+    s = psi / W.PSI0
+    B = W.B0 * (1 + sp.Rational(1, 10) * sp.sqrt(s) * sp.cos(th) + sp.Rational(1, 20) * sp.sqrt(s) * sp.cos(th - 4 * ze))
+    G = W.G0 * (1 + sp.Rational(1, 20) * s - sp.Rational(1, 50) * s ** 2)
+    I = W.G0 * (sp.Rational(1, 50) * s + sp.Rational(1, 100) * s ** 3)
+    iota = sp.Rational(42, 100) + sp.Rational(1, 10) * s + sp.Rational(1, 20) * s ** 2
+    psi_p = W.PSI0 * sp.integrate(iota.subs(psi, sp.Symbol("x") * W.PSI0), (sp.Symbol("x"), 0, s))
+    rho = M * v / (Q * B)
+    z = [psi, th, ze, v]
+    A = [sp.Integer(0), Q * (psi + rho * I), Q * (rho * G - psi_p), sp.Integer(0)]
+    H = M * v ** 2 / 2 + M * mu * B
+    Om = sp.Matrix(4, 4, lambda i, j: sp.diff(A[i], z[j]) - sp.diff(A[j], z[i]))
+    rhs = sp.Matrix([-sp.diff(H, z[i]) for i in range(4)])
+    fOm = sp.lambdify((psi, th, ze, v, mu), Om, "numpy")
+    frhs = sp.lambdify((psi, th, ze, v, mu), rhs, "numpy")
+    fB = sp.lambdify((psi, th, ze), [B, sp.diff(B, psi) * W.PSI0, sp.diff(B, th), sp.diff(B, ze)], "numpy")
+    f = O.Field(_nonvacuum_fd())
+    p = O.make_params(W.base_params(1e-4))
+    rng = np.random.default_rng(29)
+    for _ in range(25):
+        s_ = 0.1 + 0.8 * rng.random()
+        th_, ze_ = 2 * math.pi * rng.random(), 2 * math.pi * rng.random()
+        v_ = (2 * rng.random() - 1) * W.V_TOTAL
+        fv = np.array(fB(s_ * W.PSI0, th_, ze_), dtype=float)
+        mu_ = (W.V_TOTAL ** 2 - v_ ** 2) / (2 * fv[0])
+        got = O.gc_boozer(f, p, mu_, 0.0, s_, th_, ze_, v_, fv)
+        want = np.linalg.solve(np.array(fOm(s_ * W.PSI0, th_, ze_, v_, mu_), dtype=float),
+                               np.array(frhs(s_ * W.PSI0, th_, ze_, v_, mu_), dtype=float).ravel())
+        want[0] /= W.PSI0
+        scale = np.array([1e5, 1e6, 1e6, 1e12])
+        assert np.all(np.abs(got - want) <= 1e-9 * np.maximum(np.abs(want), 1e-6 * scale)), (got, want)
+
+
+def test_nonvacuum_reduces_to_vacuum(oracle):
+    """Constant G, I = 0 and the linear iota given as PROFILES give the vacuum right-hand side R1."""
+    O = oracle
+    fd = _boozer_fd()
+    sn = np.linspace(0.0, 1.0, 4)
+    fd1 = dict(fd, G_nodes=np.full(4, W.G0), I_nodes=np.zeros(4), iota_nodes=W.IOTA0 + W.IOTA1 * sn)
+    p = O.make_params(W.base_params(1e-4))
+    fv = np.array([5.5, 0.3, -0.2, 0.4])
+    a = O.gc_boozer(O.Field(fd), p, 3e12, 0.0, 0.4, 1.0, 2.0, 7e6, fv)
+    b = O.gc_boozer(O.Field(fd1), p, 3e12, 0.0, 0.4, 1.0, 2.0, 7e6, fv)
+    assert np.allclose(a, b, rtol=1e-14, atol=0)
+
+
+def test_nonvacuum_energy_and_pzeta_conserved(oracle):
+    """Invariants of R1b in an analytic axisymmetric field B(s, theta): energy v^2/2 + mu B and the canonical toroidal
+    momentum P_zeta = rho G - psi_p (per unit charge), along a traced orbit."""
+    O = oracle
+
+    def fn(x):
+        s, th = max(x[0], 1e-12), x[1]
+        r = math.sqrt(s)
+        return [W.B0 * (1 + 0.1 * r * math.cos(th)), W.B0 * 0.05 / r * math.cos(th), -W.B0 * 0.1 * r * math.sin(th), 0.0]
+
+    f = O.Field(_nonvacuum_fd(), analytic=fn)
+    p = O.make_params(W.base_params(2e-5, rtol=1e-10, atol=1e-13))
+    x0 = np.array([[0.3, 0.5], [0.4, 2.0], [0.1, 1.0], [0.6 * W.V_TOTAL, -0.3 * W.V_TOTAL]])
+    r = O.trace(f, p, x0)
+    assert np.all(r["status"] == 0)
+
+    def invariants(x):
+        s, th, v = x[0], x[1], x[3]
+        B = np.array([fn([s[i], th[i], 0.0])[0] for i in range(len(s))])
+        B0v = np.array([fn([x0[0][i], x0[1][i], 0.0])[0] for i in range(len(s))])
+        muv = (W.V_TOTAL ** 2 - x0[3] ** 2) / (2 * B0v)
+        E = 0.5 * v ** 2 + muv * B
+        psi_p = W.PSI0 * (0.42 * s + 0.05 * s ** 2 + 0.05 * s ** 3 / 3)
+        Pz = (M * v / (Q * B)) * _NV_G(s) - psi_p
+        return E, Pz
+
+    E0, P0 = invariants(x0)
+    E1, P1 = invariants(r["xf"])
+    assert np.all(np.abs(E1 / E0 - 1) < 1e-8)
+    assert np.all(np.abs(P1 - P0) < 1e-8 * W.PSI0)

@@ -55,15 +55,19 @@ UNIT = "accepted steps/s"
 # exp / division = 1 flop each): ~100 (Boozer vacuum), ~150 (Boozer + wave), ~120 (Cartesian); per attempted step
 # ~150 flops of stage / error algebra.  `roofline.achieved` and `roofline.frac` use these.
 ALG_FLOPS_PER_EVAL = {"boozer_vac": 4 * 168 + 30 + 100, "boozer_saw": 4 * 168 + 30 + 150, "cart": 7 * 168 + 30 + 120}
+# derivative-of-interpolant mode (R1c; not one of SURVEY 8(d)'s figures): value and gradient of ONE tricubic by
+# the simultaneous value / derivative Horner scheme, 112 FMA, + locate and right-hand side as above
+ALG_FLOPS_PER_EVAL.update({"boozer_vac_doi": 224 + 100, "boozer_saw_doi": 224 + 150})
 ALG_FLOPS_PER_ATTEMPT = 150
 # EXECUTED work of the tracer kernels (their own arithmetic: 63-FMA Horner per quantity in the monomial basis, no
 # Lagrange basis; the scalar warp's and the stage sums' DFMA / DMUL / DADD per evaluation from the ncu instruction mix
 # of the committed capture, profiles/r2_ncu_trace_pair.md: 391 DFMA + 75 DMUL + 22 DADD thread instructions per
 # evaluation, lanes without a particle included).  `roofline.executed` uses these; stage algebra included.
 EXEC_FLOPS_PER_EVAL = {"boozer_vac": 4 * 126 + 275, "boozer_saw": 4 * 126 + 375, "cart": 7 * 126 + 260}
+EXEC_FLOPS_PER_EVAL.update({"boozer_vac_doi": 224 + 290, "boozer_saw_doi": 224 + 390})
 # particle slots served by one thread block (tracer_pair.cu: two warp pairs; tracer.cu: one scalar warp)
-SLOTS_PER_BLOCK = {"boozer_vac": 64, "boozer_saw": 64, "cart": 32}
-BYTES_PER_CELL_VISIT = {"boozer_vac": 4 * 512, "boozer_saw": 4 * 512, "cart": 7 * 512}
+SLOTS_PER_BLOCK = {"boozer_vac": 64, "boozer_saw": 64, "cart": 32, "boozer_vac_doi": 64, "boozer_saw_doi": 64}
+BYTES_PER_CELL_VISIT = {"boozer_vac": 4 * 512, "boozer_saw": 4 * 512, "cart": 7 * 512, "boozer_vac_doi": 512, "boozer_saw_doi": 512}
 KERNELS_PER_STEP = {"catapult_field_build": 1, "catapult_trace_continue": 1, "catapult_trace": 1, "catapult_estimate": 2}
 
 
@@ -222,6 +226,8 @@ def main():
     ap.add_argument("--particles", type=int, default=0, help="particles per GPU (0 = the config's full size)")
     ap.add_argument("--cells", type=int, default=0, help="cells per dimension of the same field (0 = the config's grid): "
                     "the grid-resolution axis of the paper's sweeps (PAPER.md:100-102)")
+    ap.add_argument("--derivative-of-interpolant", action="store_true", help="Boozer configs: tabulate |B| only (nquant = 1) and "
+                    "take its derivatives from the interpolant (DESIGN.md R1c, SURVEY 8(f) f2): a quarter of the table")
     ap.add_argument("--rtol", type=float, default=0.0, help="tracing tolerance (0 = the config's 1e-9): PAPER.md:100-102")
     ap.add_argument("--e2e-steps", type=int, default=-1, help="steps of the host-buffer leg (-1 = --steps, 0 = skip)")
     ap.add_argument("--job-particles", type=int, default=65536,
@@ -272,8 +278,12 @@ def main():
     cfg = W.config(cfg_idx, n=per_gpu * world, ncell=ncell)          # ONE ensemble of world x per_gpu particles
     if args.rtol > 0:
         cfg["params"]["rtol"] = args.rtol
+    if args.derivative_of_interpolant:
+        if cfg["field"]["coord"] != 0:
+            raise SystemExit("--derivative-of-interpolant is a Boozer mode")
+        cfg["field"] = dict(cfg["field"], nquant=1, nodes=np.ascontiguousarray(cfg["field"]["nodes"][:1]))
     fd, pd = cfg["field"], cfg["params"]
-    model = model_of(cfg)
+    model = model_of(cfg) + ("_doi" if args.derivative_of_interpolant else "")
     x0 = S.shard_columns(cfg["x0"], rank, world)                     # this rank's share: rank, rank + world, ...
     npart = x0.shape[1]
     d_nodes = torch.from_numpy(fd["nodes"]).cuda()

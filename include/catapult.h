@@ -51,6 +51,10 @@ typedef enum {
    Cylindrical grid (R3): B_R, B_phi, B_Z, d|B|/dR, (1/R) d|B|/dphi, d|B|/dZ,
                                     psi (loss level function)        -> nquant = 7 */
 #define CATAPULT_NQUANT_BOOZER 4
+/* Boozer, derivative-of-interpolant mode (R1c): only |B| is tabulated (nquant = 1, one 512-byte block per
+   cell instead of four); d|B|/ds, d|B|/dtheta, d|B|/dzeta are the derivatives of its local tricubic.  The right-hand
+   side then jumps at cell faces: more and more often rejected steps than with tabulated derivative columns. */
+#define CATAPULT_NQUANT_BOOZER_DOI 1
 #define CATAPULT_NQUANT_CYL 7
 
 /* semantic tags of the columns (catapult_field_desc.quant).  All sixteen entries zero = the canonical
@@ -78,7 +82,7 @@ typedef struct {
   int32_t ncell[3]; /* interpolant cells per dimension, slowest -> fastest;
                        unique nodes per dimension = 3*ncell+1 */
   int32_t nfp;      /* field periods: the last grid dimension spans [lo, lo + 2pi/nfp) */
-  int32_t nquant;   /* m, must equal CATAPULT_NQUANT_* of `coord` */
+  int32_t nquant;   /* m, must equal CATAPULT_NQUANT_* of `coord` (Boozer: 4, or 1 = derivative-of-interpolant mode) */
   int32_t quant[16]; /* CATAPULT_Q_* tag of every column, or all zero (= the canonical order of `coord`) */
   double lo[3], hi[3]; /* Boozer: [0,1],[0,2pi],[0,2pi/nfp]; cyl: [Rmin,Rmax],[Zmin,Zmax],[0,2pi/nfp].
                           theta, zeta and phi are periodic with period hi-lo; s, R, Z extrapolate

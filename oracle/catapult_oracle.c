@@ -116,6 +116,37 @@ void orc_tricubic(const orc_field *f, const double x[3], double *out) {
   }
 }
 
+/* DESIGN.md reading R1c: the gradient of the SAME local tricubic, obtained by differentiating the
+   Lagrange basis along one axis at a time; d/dx_d = (d/du_d) / h_d. */
+void orc_tricubic_grad(const orc_field *f, const double x[3], int q, double *val, double grad[3]) {
+  int32_t cell[3];
+  double u[3], L[3][4], dL[3][4];
+  orc_locate(f, x, cell, u);
+  for (int d = 0; d < 3; ++d) {
+    orc_lagrange4(u[d], L[d]);
+    orc_dlagrange4(u[d], dL[d]);
+  }
+  const int64_t n0 = 3 * (int64_t)f->ncell[0] + 1, n1 = 3 * (int64_t)f->ncell[1] + 1,
+                n2 = 3 * (int64_t)f->ncell[2] + 1;
+  const double *F = f->nodes + (int64_t)q * n0 * n1 * n2;
+  double v = 0.0, g0 = 0.0, g1 = 0.0, g2 = 0.0;
+  for (int a = 0; a < 4; ++a)
+    for (int b = 0; b < 4; ++b)
+      for (int c = 0; c < 4; ++c) {
+        const int64_t j0 = 3 * (int64_t)cell[0] + a, j1 = 3 * (int64_t)cell[1] + b, j2 = 3 * (int64_t)cell[2] + c;
+        const double Fv = F[(j0 * n1 + j1) * n2 + j2];
+        v += L[0][a] * L[1][b] * L[2][c] * Fv;
+        g0 += dL[0][a] * L[1][b] * L[2][c] * Fv;
+        g1 += L[0][a] * dL[1][b] * L[2][c] * Fv;
+        g2 += L[0][a] * L[1][b] * dL[2][c] * Fv;
+      }
+  *val = v;
+  for (int d = 0; d < 3; ++d) {
+    const double h = (f->hi[d] - f->lo[d]) / (double)f->ncell[d];
+    grad[d] = (d == 0 ? g0 : (d == 1 ? g1 : g2)) / h;
+  }
+}
+
 void orc_tricubic_many(const orc_field *f, int64_t npts, const double *pts, double *out) {
   for (int64_t i = 0; i < npts; ++i) {
     double x[3] = {pts[i], pts[npts + i], pts[2 * npts + i]};
@@ -271,7 +302,13 @@ void orc_rhs(const orc_field *f, const orc_params *p, double mu, double t, const
     const double s = sqrt(y[0] * y[0] + y[1] * y[1]);
     const double theta = atan2(y[1], y[0]);
     const double x[3] = {s, theta, y[2]};
-    orc_tricubic(f, x, fv);
+    if (f->nquant == 1 && !f->analytic) {
+      /* reading R1c (derivative-of-interpolant mode): only |B| is tabulated, its derivatives are those of its
+         interpolant */
+      orc_tricubic_grad(f, x, 0, &fv[0], &fv[1]);
+    } else {
+      orc_tricubic(f, x, fv);
+    }
     orc_gc_boozer(f, p, mu, t, s, theta, y[2], y[3], fv, d);
     /* d/dt (s cos th, s sin th) with cos th = y0/s, sin th = y1/s */
     const double c = (s > 0.0) ? y[0] / s : 1.0, sn = (s > 0.0) ? y[1] / s : 0.0;
@@ -285,7 +322,7 @@ void orc_rhs(const orc_field *f, const orc_params *p, double mu, double t, const
     orc_tricubic(f, x, fv);
     orc_gc_cartesian(p, mu, y, y[3], fv, dy);
   }
-  if (fv_out) memcpy(fv_out, fv, sizeof(double) * (size_t)f->nquant);
+  if (fv_out) memcpy(fv_out, fv, sizeof(double) * (size_t)(f->nquant == 1 ? 4 : f->nquant));
 }
 
 /* ------------------------------------------------------------------------------------------

@@ -102,6 +102,9 @@ void orc_profile(const orc_field *f, const double *nodes, double s, double *val,
 void orc_lagrange4(double u, double L[4]);
 void orc_locate(const orc_field *f, const double x[3], int32_t cell[3], double u[3]);
 void orc_tricubic(const orc_field *f, const double x[3], double *out /*[m]*/);
+/* value and gradient (with respect to the three grid coordinates) of quantity q's interpolant: the local tricubic of
+   PAPER.md:47-53 differentiated (reading R1c, the derivative-of-interpolant mode) */
+void orc_tricubic_grad(const orc_field *f, const double x[3], int q, double *val, double grad[3]);
 void orc_tricubic_many(const orc_field *f, int64_t npts, const double *pts /*[3][npts]*/,
                        double *out /*[m][npts]*/);
 /* paper's stored layout D1: out[((cell*64)+node)*m + q], cell and node ordered dim0,dim1,dim2

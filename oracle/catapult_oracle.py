@@ -182,7 +182,7 @@ def rhs(f: Field, p: CParams, mu, t, y):
     dy = np.zeros(4)
     fv = np.zeros(16)
     lib().orc_rhs(f.ref, C.byref(p), C.c_double(mu), C.c_double(t), _dp(y), _dp(dy), _dp(fv))
-    return dy, fv[: f.c.nquant].copy()
+    return dy, fv[: (4 if f.c.nquant == 1 else f.c.nquant)].copy()
 
 
 def dp5_tableau():
@@ -289,6 +289,14 @@ def trace_scripted(f: Field, p: CParams, x0, h):
     n = lib().orc_trace_scripted(f.ref, C.byref(p), _dp(x0), C.c_int64(h.size), _dp(h), _dp(xf),
                                  C.byref(ts), C.byref(st), _dp(r))
     return xf, ts.value, st.value, r[:n].copy()
+
+
+def tricubic_grad(f: Field, x, q: int = 0):
+    """value and gradient (d/dx0, d/dx1, d/dx2) of quantity q's interpolant at x (reading R1c)"""
+    v = C.c_double(0)
+    g = np.zeros(3)
+    lib().orc_tricubic_grad(f.ref, _dp(_f64(x)), C.c_int(q), C.byref(v), _dp(g))
+    return v.value, g
 
 
 def profile(f: Field, nodes, s: float):

@@ -42,8 +42,12 @@ static catapult_status validate_desc(const catapult_field_desc* d) {
     ncells *= d->ncell[i];
     if (ncells > (long long)INT32_MAX) return fail(CATAPULT_EINVAL, "desc.ncell: more than 2^31-1 cells");
   }
-  const int want = d->coord == CATAPULT_COORD_BOOZER ? CATAPULT_NQUANT_BOOZER : CATAPULT_NQUANT_CYL;
-  if (d->nquant != want) return fail(CATAPULT_EINVAL, "desc.nquant does not match desc.coord (4 Boozer, 7 cyl)");
+  // Boozer with ONE quantity: the derivative-of-interpolant mode (only |B| tabulated, R1c)
+  const bool doi = d->coord == CATAPULT_COORD_BOOZER && d->nquant == CATAPULT_NQUANT_BOOZER_DOI;
+  const int want = doi ? CATAPULT_NQUANT_BOOZER_DOI
+                       : (d->coord == CATAPULT_COORD_BOOZER ? CATAPULT_NQUANT_BOOZER : CATAPULT_NQUANT_CYL);
+  if (d->nquant != want)
+    return fail(CATAPULT_EINVAL, "desc.nquant does not match desc.coord (Boozer: 4, or 1 = derivative-of-interpolant mode; cyl: 7)");
   // semantic tags of the columns: all zero = the canonical order of `coord`; anything else must spell it out
   bool tagged = false;
   for (int i = 0; i < 16; ++i) tagged = tagged || d->quant[i] != 0;

@@ -46,7 +46,7 @@ struct PairTraits {
   // one slot's run of shared memory: NSH doubles + 16 bytes of padding, so that the 8 lanes of a quarter warp
   // reading 16 bytes each at the same offset of their runs hit 8 different 16-byte bank groups (STRIP/16 is odd)
   static constexpr int STRIP = NSH * 8 + 16;
-  static_assert(NREG % 4 == 0 && NREG > 0 && NREG < NCOEF, "register part: whole rows");
+  static_assert(NREG >= 64 && NREG % 4 == 0 && NREG > 0 && NREG < NCOEF, "register part: whole rows");
   static_assert((STRIP / 16) % 2 == 1, "run length must be an odd number of 16-byte groups");
   static constexpr size_t OFF_COEF = 0;                               // [NS] runs of STRIP bytes
   static constexpr size_t OFF_MBAR = OFF_COEF + (size_t)STRIP * NS;   // uint64 [NS]: one mbarrier per slot
@@ -85,9 +85,17 @@ __device__ __forceinline__ void pair_wait(PairCell& pc) {
 // Fetch of cell c: the first NREG coefficients land in their final registers (256-bit loads), the others go
 // global -> shared as ONE bulk asynchronous copy.  Nothing waits here, except for an earlier copy that is still
 // landing in the same run.
+template <bool DOI>
 __device__ __forceinline__ void pair_fetch(const double* __restrict__ table, PairCell& pc,
                                            double (&creg)[PairTraits::NREG], int c) {
   using PT = PairTraits;
+  if (DOI) {  // one quantity: 512 bytes, all of it into registers
+    const double* src1 = table + (long long)c * 64;
+#pragma unroll
+    for (int e = 0; e < 64; e += 4) ldg_f64x4(src1 + e, creg[e], creg[e + 1], creg[e + 2], creg[e + 3]);
+    pc.cached = c;
+    return;
+  }
   const double* src = table + (long long)c * PT::NCOEF;
 #pragma unroll
   for (int e = 0; e < PT::NREG; e += 4) ldg_f64x4(src + e, creg[e], creg[e + 1], creg[e + 2], creg[e + 3]);
@@ -186,6 +194,41 @@ __device__ __forceinline__ void pair_contract(const double (&creg)[PairTraits::N
   }
 }
 
+// Derivative-of-interpolant mode (R1c): ONE tabulated quantity, |B|, whose 64 coefficients all sit in the
+// thread's registers; the contraction delivers, per power a of wLAST, the plane value, its derivative with respect to
+// wSECOND and the plane value of the rows' derivatives with respect to wFIRST (simultaneous value / derivative Horner:
+// p <- c3, d <- c3; then d <- d w + p after every p <- p w + c).  112 FMA, no shared-memory traffic.
+__device__ __forceinline__ void pair_contract_doi(const double (&creg)[PairTraits::NREG], unsigned part_s, double wS,
+                                                  double wF) {
+  using PT = PairTraits;
+#pragma unroll
+  for (int a = 0; a < 4; ++a) {
+    double V = 0.0, VS = 0.0, VF = 0.0;
+#pragma unroll
+    for (int b = 3; b >= 0; --b) {
+      const int g = (a * 4 + b) * 4;
+      double r = creg[g + 3], dr = creg[g + 3];
+      r = fma(r, wF, creg[g + 2]);
+      dr = fma(dr, wF, r);
+      r = fma(r, wF, creg[g + 1]);
+      dr = fma(dr, wF, r);
+      r = fma(r, wF, creg[g]);
+      if (b == 3) {
+        V = r;
+        VS = r;
+        VF = dr;
+      } else {
+        V = fma(V, wS, r);
+        if (b > 0) VS = fma(VS, wS, V);
+        VF = fma(VF, wS, dr);
+      }
+    }
+    sts_f64x2(part_s + (unsigned)((a * 2 + 0) * PT::NS) * 16u, V, VS);
+    sts_f64x2(part_s + (unsigned)((a * 2 + 1) * PT::NS) * 16u, VF, 0.0);
+  }
+}
+
+template <bool DOI>
 __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned char* smem, int slot, int bar0) {
   using PT = PairTraits;
   const unsigned FULL = 0xffffffffu;
@@ -213,7 +256,7 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
     // first quads need (neither depends on the evaluation point), so that the request finds the thread ready
     pair_wait(pc);
     if (__double2hiint(creg[PT::NREG - 1]) == 0x7ffdead0) asm volatile("nanosleep.u32 1;");  // = wait for the loads
-    rows.preload(pc.strip_s);
+    if (!DOI) rows.preload(pc.strip_s);
     pbar_sync(bar0 + PB_REQ);
     const int rq = reqbuf[0];
     if (rq & REQ_QUIT) {  // pair-uniform
@@ -224,7 +267,10 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
     const int kind = (rq >> 1) & 7;  // pair-uniform
     const int rpar = (rq >> 6) & 1;
     const double wF = wbuf[0], wS = wbuf[PT::NS];
-    if (active) pair_contract(creg, rows, pc.strip_s, part_s, wS, wF);
+    if (active) {
+      if (DOI) pair_contract_doi(creg, part_s, wS, wF);
+      else pair_contract(creg, rows, pc.strip_s, part_s, wS, wF);
+    }
     __syncwarp();
     pbar_arrive(bar0 + PB_DONE);
     // ---- the scalar warp has located the point: a wrong cell is redone; then the guessed cell of the next
@@ -235,26 +281,31 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
     const bool redo = active && redo_cell >= 0;
     if (__any_sync(FULL, redo)) {  // the scalar warp takes the same decision
       if (redo) {
-        pair_fetch(table, pc, creg, redo_cell);
-        pair_wait(pc);
-        rows.preload(pc.strip_s);
-        pair_contract(creg, rows, pc.strip_s, part_s, wS, wF);
+        pair_fetch<DOI>(table, pc, creg, redo_cell);
+        if (DOI) {
+          pair_contract_doi(creg, part_s, wS, wF);
+        } else {
+          pair_wait(pc);
+          rows.preload(pc.strip_s);
+          pair_contract(creg, rows, pc.strip_s, part_s, wS, wF);
+        }
       }
       __syncwarp();
       pbar_arrive(bar0 + PB_D2);
     }
-    if (active && next_cell >= 0 && next_cell != pc.cached) pair_fetch(table, pc, creg, next_cell);
+    if (active && next_cell >= 0 && next_cell != pc.cached) pair_fetch<DOI>(table, pc, creg, next_cell);
     if (kind == 5) {  // end of an attempt: the first point of the next one depends on the accept / reject decision
       pbar_sync(bar0 + PB_G2);
       const long long g2 = g2buf[0];
       const int t2 = (int)g2, far = (int)(g2 >> 32);
-      if (active && t2 >= 0 && t2 != pc.cached) pair_fetch(table, pc, creg, t2);
+      if (active && t2 >= 0 && t2 != pc.cached) pair_fetch<DOI>(table, pc, creg, t2);
       // the cell in which the next attempt is expected to end: towards L2 now (30 % of the fetches come from
       // HBM otherwise, and a warp waits for its slowest lane)
       if (active && far >= 0 && far != pc.cached) {
-        const char* line = reinterpret_cast<const char*>(table + (long long)far * PT::NCOEF);
+        constexpr int CELL_DOUBLES = DOI ? 64 : PT::NCOEF;
+        const char* line = reinterpret_cast<const char*>(table + (long long)far * CELL_DOUBLES);
 #pragma unroll
-        for (int l = 0; l < PT::NCOEF * 8 / 128; ++l) asm volatile("prefetch.global.L2 [%0];" ::"l"(line + 128 * l));
+        for (int l = 0; l < CELL_DOUBLES * 8 / 128; ++l) asm volatile("prefetch.global.L2 [%0];" ::"l"(line + 128 * l));
       }
     }
   }
@@ -287,7 +338,7 @@ struct ScalarSide {  // what the scalar warp carries from round to round besides
 // Lanes with act = false publish a request nobody serves.  ratio >= 0: the next point is expected at
 // X + ratio (X - base) and its cell is fetched ahead.  S_c = sum_{j < 6} coef[j] k_j,c is accumulated on the side
 // (rows of PAIR_SUMS).  All 32 lanes must call this.
-template <int MODEL>
+template <int MODEL, bool DOI>
 __device__ __forceinline__ void scalar_round(const TraceConst& tc, unsigned char* smem, int slot, int bar0, bool act,
                                              int kind, ScalarSide& sr, double tr, const double X[4], double mu,
                                              float ratio, const float base[3], float pos[3], double dy[4],
@@ -376,15 +427,26 @@ __device__ __forceinline__ void scalar_round(const TraceConst& tc, unsigned char
       p[a][0] = part[(a * 2 + 0) * PT::NS];
       p[a][1] = part[(a * 2 + 1) * PT::NS];
     }
-    fv[0] = horner_row(p[0][0].x, p[1][0].x, p[2][0].x, p[3][0].x, wL);
-    fv[1] = horner_row(p[0][0].y, p[1][0].y, p[2][0].y, p[3][0].y, wL);
-    fv[2] = horner_row(p[0][1].x, p[1][1].x, p[2][1].x, p[3][1].x, wL);
-    fv[3] = horner_row(p[0][1].y, p[1][1].y, p[2][1].y, p[3][1].y, wL);
+    if (DOI) {
+      // reading R1c: |B| and its gradient from ONE interpolant; d/dx = (d/dw) 2 / h (w = 2 u - 1)
+      fv[0] = horner_row(p[0][0].x, p[1][0].x, p[2][0].x, p[3][0].x, wL);
+      const double dL = fma(fma(3.0 * p[3][0].x, wL, 2.0 * p[2][0].x), wL, p[1][0].x);
+      const double dS = horner_row(p[0][0].y, p[1][0].y, p[2][0].y, p[3][0].y, wL);
+      const double dF = horner_row(p[0][1].x, p[1][1].x, p[2][1].x, p[3][1].x, wL);
+      fv[1] = dS * (2.0 * f.invh[AX::SECOND]);
+      fv[2] = dL * (2.0 * f.invh[AX::LAST]);
+      fv[3] = dF * (2.0 * f.invh[AX::FIRST]);
+    } else {
+      fv[0] = horner_row(p[0][0].x, p[1][0].x, p[2][0].x, p[3][0].x, wL);
+      fv[1] = horner_row(p[0][0].y, p[1][0].y, p[2][0].y, p[3][0].y, wL);
+      fv[2] = horner_row(p[0][1].x, p[1][1].x, p[2][1].x, p[3][1].x, wL);
+      fv[3] = horner_row(p[0][1].y, p[1][1].y, p[2][1].y, p[3][1].y, wL);
+    }
   }
   eval_physics<MODEL>(tc, X, mu, g, fv, dy, modB, level);
 }
 
-template <int MODEL, int MODE>
+template <int MODEL, int MODE, bool DOI>
 __global__ void __launch_bounds__(PairTraits::NT, 2)
 trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ TraceArgs a, const int lane_cap) {
   using PT = PairTraits;
@@ -407,7 +469,7 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
   const int slot = pair * 32 + lane;
   const int bar0 = 1 + 6 * pair;
   if ((warp >> 1) != flip) {
-    contraction_warp(tc, smem, slot, bar0);
+    contraction_warp<DOI>(tc, smem, slot, bar0);
     return;
   }
   const unsigned FULL = 0xffffffffu;
@@ -510,7 +572,7 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
       // the start point's field values give mu and k1
       double dy0[4], B, level, S[4];
       float pos[3];
-      scalar_round<MODEL>(tc, smem, slot, bar0, fresh, KIND_START, sr, t, y, 0.0, -1.f, base, pos, dy0, B, level,
+      scalar_round<MODEL, DOI>(tc, smem, slot, bar0, fresh, KIND_START, sr, t, y, 0.0, -1.f, base, pos, dy0, B, level,
                           PAIR_SUMS[6], ks, S);
       ++rounds;
       if (fresh) {
@@ -548,7 +610,7 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
       // once per particle)
       const bool go = fresh && active;
       if (__any_sync(FULL, go)) {
-        scalar_round<MODEL>(tc, smem, slot, bar0, go, KIND_START, sr, t, y, mu, -1.f, base, pos, dy0, B, level,
+        scalar_round<MODEL, DOI>(tc, smem, slot, bar0, go, KIND_START, sr, t, y, mu, -1.f, base, pos, dy0, B, level,
                             PAIR_SUMS[6], ks, S);
         ++rounds;
         if (go) {
@@ -605,7 +667,7 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
         const float ratio = (MODE == MODE_STEP_ONCE && r == 5) ? -1.f : NEXT_POINT_RATIO[r];
         // on the side: the known part of the next stage state; in the last round the error sums of Eq. 4
         // over the first six derivatives
-        scalar_round<MODEL>(tc, smem, slot, bar0, stepping, r, sr, fma(DP_C[r], h, t), X, mu, ratio, base, pos, dy, B_,
+        scalar_round<MODEL, DOI>(tc, smem, slot, bar0, stepping, r, sr, fma(DP_C[r], h, t), X, mu, ratio, base, pos, dy, B_,
                             level, PAIR_SUMS[r], ks, S);
         if (r < 5) {  // k_7 stays in registers: it is the next step's k_1 (or nothing)
 #pragma unroll
@@ -738,7 +800,7 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
 
 // ---- launchers ---------------------------------------------------------------------------------------------
 // Persistent grid: two blocks per SM (or fewer when there are fewer particles than warps could share out).
-template <int MODEL, int MODE>
+template <int MODEL, int MODE, bool DOI>
 static catapult_status pair_shape(int64_t n, int* blocks, int* threads, int* lane_cap) {
   using PT = PairTraits;
   static thread_local int cached_device = -1, cached_resident = 0;
@@ -747,9 +809,9 @@ static catapult_status pair_shape(int64_t n, int* blocks, int* threads, int* lan
   if (cached_device != dev) {
     int sms = 0, per_sm = 0;
     CATAPULT_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CATAPULT_CUDA_TRY(cudaFuncSetAttribute(trace_pair_kernel<MODEL, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    CATAPULT_CUDA_TRY(cudaFuncSetAttribute(trace_pair_kernel<MODEL, MODE, DOI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            (int)PT::SMEM_BYTES));
-    CATAPULT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_pair_kernel<MODEL, MODE>, PT::NT,
+    CATAPULT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_pair_kernel<MODEL, MODE, DOI>, PT::NT,
                                                                     PT::SMEM_BYTES));
     if (per_sm < 1) {
       set_error("the tracer kernel does not fit on this device (registers / shared memory)");
@@ -770,12 +832,12 @@ static catapult_status pair_shape(int64_t n, int* blocks, int* threads, int* lan
   return CATAPULT_OK;
 }
 
-template <int MODEL, int MODE>
+template <int MODEL, int MODE, bool DOI>
 static catapult_status pair_launch(const TraceConst& tc, const TraceArgs& a, cudaStream_t s) {
   int blocks = 0, threads = 0, cap = 32;
-  catapult_status st = pair_shape<MODEL, MODE>(a.n, &blocks, &threads, &cap);
+  catapult_status st = pair_shape<MODEL, MODE, DOI>(a.n, &blocks, &threads, &cap);
   if (st != CATAPULT_OK) return st;
-  trace_pair_kernel<MODEL, MODE><<<blocks, threads, PairTraits::SMEM_BYTES, s>>>(tc, a, cap);
+  trace_pair_kernel<MODEL, MODE, DOI><<<blocks, threads, PairTraits::SMEM_BYTES, s>>>(tc, a, cap);
   CATAPULT_CUDA_TRY(cudaGetLastError());
   return CATAPULT_OK;
 }
@@ -783,9 +845,14 @@ static catapult_status pair_launch(const TraceConst& tc, const TraceArgs& a, cud
 template <int MODE>
 static catapult_status pair_dispatch(const TraceConst& tc, const TraceArgs& a, int model, cudaStream_t s) {
   if (a.n == 0) return CATAPULT_OK;
-  if (model == MODEL_BOOZER_VAC) return pair_launch<MODEL_BOOZER_VAC, MODE>(tc, a, s);
-  if (model == MODEL_BOOZER_NV) return pair_launch<MODEL_BOOZER_NV, MODE>(tc, a, s);
-  return pair_launch<MODEL_BOOZER_SAW, MODE>(tc, a, s);
+  if (tc.f.m == 1) {  // derivative-of-interpolant mode (one tabulated quantity)
+    if (model == MODEL_BOOZER_VAC) return pair_launch<MODEL_BOOZER_VAC, MODE, true>(tc, a, s);
+    if (model == MODEL_BOOZER_NV) return pair_launch<MODEL_BOOZER_NV, MODE, true>(tc, a, s);
+    return pair_launch<MODEL_BOOZER_SAW, MODE, true>(tc, a, s);
+  }
+  if (model == MODEL_BOOZER_VAC) return pair_launch<MODEL_BOOZER_VAC, MODE, false>(tc, a, s);
+  if (model == MODEL_BOOZER_NV) return pair_launch<MODEL_BOOZER_NV, MODE, false>(tc, a, s);
+  return pair_launch<MODEL_BOOZER_SAW, MODE, false>(tc, a, s);
 }
 
 catapult_status launch_trace_pair(const TraceConst& tc, const TraceArgs& a, int model, int mode, cudaStream_t s) {
@@ -798,9 +865,9 @@ catapult_status launch_trace_pair(const TraceConst& tc, const TraceArgs& a, int 
 
 catapult_status trace_pair_shape(int model, int64_t n, int* blocks, int* threads) {
   int cap = 0;
-  if (model == MODEL_BOOZER_VAC) return pair_shape<MODEL_BOOZER_VAC, MODE_ADAPTIVE>(n, blocks, threads, &cap);
-  if (model == MODEL_BOOZER_NV) return pair_shape<MODEL_BOOZER_NV, MODE_ADAPTIVE>(n, blocks, threads, &cap);
-  return pair_shape<MODEL_BOOZER_SAW, MODE_ADAPTIVE>(n, blocks, threads, &cap);
+  if (model == MODEL_BOOZER_VAC) return pair_shape<MODEL_BOOZER_VAC, MODE_ADAPTIVE, false>(n, blocks, threads, &cap);
+  if (model == MODEL_BOOZER_NV) return pair_shape<MODEL_BOOZER_NV, MODE_ADAPTIVE, false>(n, blocks, threads, &cap);
+  return pair_shape<MODEL_BOOZER_SAW, MODE_ADAPTIVE, false>(n, blocks, threads, &cap);
 }
 
 }  // namespace catapult

@@ -864,3 +864,78 @@ def test_nonvacuum_input_is_validated(K, nonvacuum_case):
     c3 = W.config(3, n=4, T=1e-6, ncell=[4, 4, 4])
     with pytest.raises(K.CatapultError):    # profiles belong to Boozer tracing
         K.catapult_field_build(dict(c3["field"], **W.nonvacuum_profiles(4)))
+
+
+# ---- f2: derivative-of-interpolant mode (one tabulated quantity, R1c) -----------------------------------
+@pytest.fixture(scope="module")
+def doi_cases(K, oracle):
+    out = {}
+    for name, idx, kw, prof in (("vac", 2, dict(n=45, T=1e-5, ncell=[12, 10, 9]), False),
+                                ("saw", 4, dict(n=33, T=1e-5, ncell=[12, 10, 9]), False),
+                                ("nv", 2, dict(n=40, T=1e-5, ncell=[12, 10, 9]), True)):
+        cfg = W.config(idx, **kw)
+        fd = dict(cfg["field"], nquant=1, nodes=np.ascontiguousarray(cfg["field"]["nodes"][:1]))
+        if prof:
+            fd.update(W.nonvacuum_profiles(12))
+        out[name] = dict(cfg=cfg, fd=fd, gf=K.catapult_field_build(fd), of=oracle.Field(fd), op=oracle.make_params(cfg["params"]))
+    return out
+
+
+@pytest.mark.parametrize("name", ["vac", "saw", "nv"])
+def test_derivative_of_interpolant_single_step_parity(K, oracle, doi_cases, name):
+    """nquant = 1: |B| and its gradient from ONE interpolant (the device differentiates the centred-monomial form,
+    the oracle the Lagrange form of the same polynomial).  One attempted step from identical state: new state to
+    1e-11, error ratio to 1e-4; the stage derivatives to 1e-10: differentiating the interpolant amplifies the ~1e-13
+    round-off of its value by |B| (2 / h) / |dB| ~ 300 (observed 3e-11).  Table a quarter of the four-column one."""
+    c = doi_cases[name]
+    cfg = c["cfg"]
+    x0 = cfg["x0"].copy()
+    n = x0.shape[1]
+    x0[0, 1::8] = 1e-3
+    x0[0, 2::8] = 0.97
+    rng = np.random.default_rng(91)
+    t = 1e-6 * rng.random(n)
+    h = cfg["params"]["dtmax"] * (0.02 + 0.1 * rng.random(n))
+    xg, rg, kg = (a.cpu().numpy() for a in K.catapult_step_once(c["gf"], cfg["params"], _dev(x0), _dev(t), _dev(h)))
+    sc = _state_scale(0)
+    worst = worst_k = worst_r = 0.0
+    for i in range(n):
+        xo, ro, ko = oracle.step_once(c["of"], c["op"], x0[:, i], t[i], h[i])
+        worst = max(worst, (np.abs(_stepped(0, xg[:, i]) - _stepped(0, xo)) / sc).max())
+        worst_k = max(worst_k, (np.abs(kg[:, :, i] - ko) / (np.abs(ko).max(axis=0)[None, :] + 1e-300)).max())
+        worst_r = max(worst_r, abs(rg[i] - ro) / max(ro, 1e-3))
+    print(f"derivative-of-interpolant ({name}) single step: state {worst:.2e}, derivatives {worst_k:.2e}, error ratio {worst_r:.2e}")
+    assert worst <= 1e-11 and worst_k <= 1e-10 and worst_r <= 1e-4
+    assert c["gf"].table_bytes * 4 == K.catapult_field_build(cfg["field"]).table_bytes
+
+
+@pytest.mark.parametrize("name", ["vac", "saw"])
+def test_derivative_of_interpolant_trajectory_parity(K, oracle, doi_cases, name):
+    """Scripted replay over 1e-5 s and the free-running adaptive run (statuses, accepted-step total).  The trajectory bar
+    is 1e-6 here, 100x the four-table mode's 1e-8: every evaluation's derivatives agree 100-300x less well (round-off
+    of the differentiated interpolant, test above), and the difference accumulates over ~1e3 steps (observed 6e-8)."""
+    c = doi_cases[name]
+    cfg = c["cfg"]
+    x0 = cfg["x0"]
+    n = x0.shape[1]
+    recs = [oracle.trace_record(c["of"], c["op"], x0[:, i]) for i in range(n)]
+    hs = [np.diff(r[0][:, 0]) for r in recs]
+    H = np.zeros((max(len(h) for h in hs) + 1, n))
+    for i, h in enumerate(hs):
+        H[:len(h), i] = h
+    g = K.catapult_trace_scripted(c["gf"], cfg["params"], _dev(x0), _dev(H))
+    gx, gt, gs = (g[k].cpu().numpy() for k in ("xf", "tstop", "status"))
+    sc = _state_scale(0)
+    worst = 0.0
+    for i in range(n):
+        xo, to, so, _ = oracle.trace_scripted(c["of"], c["op"], x0[:, i], hs[i])
+        assert gs[i] == so and gt[i] == to
+        d = _state_diff(0, gx[:, i:i + 1], xo[:, None])[:, 0]
+        worst = max(worst, (np.abs(d) / np.maximum(sc, np.abs(xo))).max())
+    print(f"derivative-of-interpolant ({name}) scripted 1e-5 s window: worst relative difference {worst:.2e}")
+    assert worst <= 1e-6
+    ga = K.catapult_trace(c["gf"], cfg["params"], _dev(x0))
+    oa = oracle.trace(c["of"], c["op"], x0)
+    assert np.array_equal(ga["status"].cpu().numpy(), oa["status"])
+    na = ga["nacc"].cpu().numpy().astype(np.int64)
+    assert abs(na.sum() - oa["nacc"].sum()) <= 0.03 * oa["nacc"].sum()

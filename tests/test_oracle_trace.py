@@ -316,3 +316,52 @@ def test_loss_time_mode_sharpens_the_loss_time(oracle):
     e0 = np.abs(loose0["tstop"][lost] - tight1["tstop"][lost])
     e1 = np.abs(loose1["tstop"][lost] - tight1["tstop"][lost])
     assert np.median(e1) < 0.05 * np.median(e0)
+
+
+def test_derivative_of_interpolant_mode(oracle):
+    """Reading R1c: only |B| tabulated, its derivatives taken from the interpolant.  (1) On a field that is one
+    tricubic polynomial per variable (one cell) the four-table mode holds the exact derivatives in its columns, so both
+    modes give the same right-hand side.  (2) On the config-0 tables the right-hand side now jumps at cell faces:
+    the controller takes more and rejects more steps (SURVEY Q2's probe), and the energy drift stays at the level of
+    the four-table mode (no better, no more than ~3x worse)."""
+    O = oracle
+    rng = np.random.default_rng(9)
+    c = 0.02 * rng.normal(size=(4, 3, 3))
+    k = [1, 1, 1]
+    lo, hi = [0.0, 0.0, 0.0], [1.0, 2 * math.pi, 2 * math.pi / 4]
+    ax = [np.linspace(lo[d], hi[d], 4) for d in range(3)]
+    P = lambda s, th, ze: W.B0 * (1 + sum(c[i, j, l] * s ** i * th ** j * ze ** l for i in range(4) for j in range(3) for l in range(3)))
+    Ps = lambda s, th, ze: W.B0 * sum(i * c[i, j, l] * s ** (i - 1) * th ** j * ze ** l for i in range(1, 4) for j in range(3) for l in range(3))
+    Pt = lambda s, th, ze: W.B0 * sum(j * c[i, j, l] * s ** i * th ** (j - 1) * ze ** l for i in range(4) for j in range(1, 3) for l in range(3))
+    Pz = lambda s, th, ze: W.B0 * sum(l * c[i, j, l] * s ** i * th ** j * ze ** (l - 1) for i in range(4) for j in range(3) for l in range(1, 3))
+    S, T, Z = np.meshgrid(*ax, indexing="ij")
+    fd4 = dict(coord=0, ncell=k, lo=lo, hi=hi, nfp=4, nquant=4, nodes=np.stack([P(S, T, Z), Ps(S, T, Z), Pt(S, T, Z), Pz(S, T, Z)]),
+               G0=W.G0, I0=0.0, iota0=W.IOTA0, iota1=W.IOTA1, psi0=W.PSI0)
+    fd1 = dict(fd4, nquant=1, nodes=fd4["nodes"][:1])
+    p = O.make_params(W.base_params(1e-5))
+    for _ in range(10):
+        s, th, ze = 0.1 + 0.8 * rng.random(), 0.2 + 5.8 * rng.random(), 0.1 + 1.3 * rng.random()
+        y = [s * math.cos(th), s * math.sin(th), ze, 0.4 * W.V_TOTAL]
+        d4, fv4 = O.rhs(O.Field(fd4), p, 3e12, 0.0, y)
+        d1, fv1 = O.rhs(O.Field(fd1), p, 3e12, 0.0, y)
+        assert np.allclose(fv1, fv4, rtol=1e-11, atol=1e-11 * W.B0)
+        assert np.allclose(d1, d4, rtol=1e-9, atol=0)
+    cfg = W.config(0, n=24, T=2e-5)
+    f4 = O.Field(cfg["field"])
+    f1 = O.Field(dict(cfg["field"], nquant=1, nodes=cfg["field"]["nodes"][:1]))
+    p = O.make_params(cfg["params"])
+    r4, r1 = O.trace(f4, p, cfg["x0"]), O.trace(f1, p, cfg["x0"])
+
+    def drift(f, r):
+        keep = r["status"] == 0
+        B0v = O.tricubic_many(f, cfg["x0"][:3])[0]
+        Bf = O.tricubic_many(f, r["xf"][:3])[0]
+        mu = (W.V_TOTAL ** 2 - cfg["x0"][3] ** 2) / (2 * B0v)
+        E = 0.5 * r["xf"][3] ** 2 + mu * Bf
+        return np.abs(E / (0.5 * W.V_TOTAL ** 2) - 1)[keep]
+
+    d4, d1 = drift(f4, r4), drift(f1, r1)
+    assert np.median(d1) < 3 * np.median(d4) + 1e-7
+    assert r1["nacc"].sum() > 1.2 * r4["nacc"].sum()          # more steps ...
+    rej = lambda r: r["nrej"].sum() / (r["nacc"].sum() + r["nrej"].sum())
+    assert rej(r1) > rej(r4)                                  # ... and more of the attempts rejected

@@ -10,6 +10,8 @@ import numpy as np
 import pytest
 from scipy.interpolate import BarycentricInterpolator
 
+from paper_2604_07617_b200 import workloads as W
+
 
 def _grid_nodes(lo, hi, ncell):
     return [lo[d] + (hi[d] - lo[d]) * np.arange(3 * ncell[d] + 1) / (3.0 * ncell[d]) for d in range(3)]
@@ -207,3 +209,45 @@ def test_field_build_bruteforce_and_size(oracle):
     for b in range(4):
         for c in range(4):
             assert np.array_equal(tab[c0 * 64 + (3 * 4 + b) * 4 + c], tab[c1 * 64 + (0 * 4 + b) * 4 + c])
+
+
+# ---- reading R1c: the gradient of the interpolant (derivative-of-interpolant mode) ---------------
+def test_gradient_of_the_interpolant_is_exact_for_tricubics(oracle):
+    """The local tricubic reproduces any polynomial of degree <= 3 per variable; so does its gradient, inside the
+    grid and where the end cells are extrapolated."""
+    O = oracle
+    rng = np.random.default_rng(5)
+    c = rng.normal(size=(4, 4, 4))
+    lo, hi, k = [0.0, -1.0, 2.0], [1.0, 1.0, 3.5], [2, 3, 2]
+    ax = [np.linspace(lo[d], hi[d], 3 * k[d] + 1) for d in range(3)]
+    P = lambda x, y, z: sum(c[i, j, l] * x ** i * y ** j * z ** l for i in range(4) for j in range(4) for l in range(4))
+    dP = lambda x, y, z: np.array([
+        sum(i * c[i, j, l] * x ** (i - 1) * y ** j * z ** l for i in range(1, 4) for j in range(4) for l in range(4)),
+        sum(j * c[i, j, l] * x ** i * y ** (j - 1) * z ** l for i in range(4) for j in range(1, 4) for l in range(4)),
+        sum(l * c[i, j, l] * x ** i * y ** j * z ** (l - 1) for i in range(4) for j in range(4) for l in range(1, 4))])
+    X, Y, Z = np.meshgrid(*ax, indexing="ij")
+    fd = dict(coord=1, ncell=k, lo=lo, hi=hi, nfp=1, nquant=1, nodes=P(X, Y, Z)[None], G0=1.0, I0=0.0, iota0=0.0,
+              iota1=0.0, psi0=1.0)        # cylindrical grid: only the last dimension is periodic
+    f = O.Field(fd)
+    for x in ([0.3, 0.1, 2.2], [0.77, -0.93, 3.4], [1.08, 1.05, 2.9], [-0.04, 0.5, 2.01]):
+        v, g = O.tricubic_grad(f, x)
+        assert abs(v - P(*x)) <= 1e-12 * (1 + abs(P(*x)))
+        assert np.all(np.abs(g - dP(*x)) <= 1e-11 * (1 + np.abs(dP(*x))))
+
+
+def test_gradient_of_the_interpolant_matches_finite_differences(oracle):
+    """On the config-0 tables: central differences of orc_tricubic (inside one cell) against orc_tricubic_grad."""
+    O = oracle
+    cfg = W.config(0, n=1, T=1e-6)
+    fd = dict(cfg["field"], nquant=1, nodes=cfg["field"]["nodes"][:1])
+    f = O.Field(fd)
+    rng = np.random.default_rng(6)
+    for _ in range(20):
+        x = np.array([0.05 + 0.9 * rng.random(), 2 * math.pi * rng.random(), 2 * math.pi / 4 * rng.random()])
+        v, g = O.tricubic_grad(f, x)
+        assert v == O.tricubic(f, x)[0]
+        for d in range(3):
+            e = np.zeros(3)
+            e[d] = 1e-6
+            fdiff = (O.tricubic(f, x + e)[0] - O.tricubic(f, x - e)[0]) / 2e-6
+            assert abs(fdiff - g[d]) <= 1e-6 * max(1.0, abs(g[d])), (d, fdiff, g[d])

@@ -1,4 +1,6 @@
-// Persistent fp64 DP5 guiding-centre tracer for the Boozer models (4 tabulated quantities): WARP PAIRS.
+// Persistent fp64 DP5 guiding-centre tracer for the Boozer models: WARP PAIRS.  Serves the vacuum model (R1), the
+// non-vacuum model with tabulated profiles (R1b) and the shear Alfven wave (R2) of DESIGN.md section 2, each with
+// four tabulated quantities or, in the derivative-of-interpolant mode (R1c, template flag DOI), with |B| alone.
 //
 // What is computed is PAPER.md:57-61 (DESIGN.md sections 1-2); the launch shape is this library's own.
 //
@@ -24,7 +26,9 @@
 // three FMA per quantity in wLAST.  The cell a contraction lane holds at REQ is the scalar warp's guess from the
 // round before (fp32 straight-line extrapolation along the attempted step; after the accept / reject decision
 // barrier G2), fetched while the scalar warp works; when the located cell differs (rare) the lane redoes the
-// contraction with the right cell (barrier D2).
+// contraction with the right cell (barrier D2).  While the scalar warp is on its own (physics, end of an attempt,
+// next stage state) the contraction warp waits for the cell that is being fetched and loads the shared-memory rows
+// of its first quad: neither depends on the evaluation point, so the request finds it ready.
 #include "tracer_common.cuh"
 
 namespace catapult {
@@ -255,7 +259,7 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
     // ---- while the scalar warp is on its own: wait for the cell that is being fetched and load the rows the
     // first quads need (neither depends on the evaluation point), so that the request finds the thread ready
     pair_wait(pc);
-    if (__double2hiint(creg[PT::NREG - 1]) == 0x7ffdead0) asm volatile("nanosleep.u32 1;");  // = wait for the loads
+    if (__double2hiint(creg[DOI ? 63 : PT::NREG - 1]) == 0x7ffdead0) asm volatile("nanosleep.u32 1;");  // = wait for the loads
     if (!DOI) rows.preload(pc.strip_s);
     pbar_sync(bar0 + PB_REQ);
     const int rq = reqbuf[0];

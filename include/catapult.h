@@ -226,6 +226,35 @@ catapult_status catapult_estimate(int32_t g_kind, int64_t n, const int32_t *d_st
                                   const double *d_tstop, const double *d_g_user, double *d_out,
                                   double *h_out, void *stream);
 
+/* ---- the estimate for callers that must not allocate device memory ------------------------------
+ * catapult_estimate above takes a few KiB of device scratch from the stream-ordered allocator on every call.
+ * Some programs cannot have a library do that on their behalf: a service that hands the whole GPU to its own
+ * memory manager at start-up and treats any later driver allocation as a bug (or simply has nothing left to
+ * give); a control loop with a latency budget, where an allocation may stall on the driver's lock or fail at
+ * the worst moment; a driver set-up without memory-pool support, where cudaMallocAsync is not available at
+ * all.  For them catapult_estimate_static computes the same four numbers -- same block partition, same
+ * summation order, so bit-identical to catapult_estimate -- and calls no cudaMalloc / cudaFree /
+ * cudaMallocAsync or any other allocating routine.  The caller passes the inputs and d_out[4] exactly as for
+ * catapult_estimate (g_kind, NULL rules and errors are the same; there is no host copy: read d_out yourself).
+ *
+ * Where the scratch lives: in a 16 KiB array that is part of libcatapult.so's device image (one pair of
+ * partial sums per block of 2048 particles).  Every GPU that loads the library carries these 16 KiB until the
+ * process exits, whether or not this function is ever called.
+ * Limit: n <= CATAPULT_ESTIMATE_STATIC_MAX_N (2,097,152 particles = 1024 blocks; twice BASELINE's largest
+ * ensemble).  A larger n is refused with CATAPULT_EINVAL and a message that names the limit; nothing is launched.
+ * First call on a device: looks up the array's address on that device (once; the current device must be the
+ * one `stream` belongs to, as for every call of this library).  Make that first call during set-up, before any
+ * stream capture is begun.
+ * Sharing: all calls on one GPU use the same array.  Calls on one stream follow each other and are safe.  Two
+ * calls that can run at the same time on one GPU (different streams, different host threads) overwrite each
+ * other's partial sums and return garbage without any error: serialise them yourself (one stream, or an event
+ * between them).  The array keeps the last call's partial sums; no call depends on them, every slot that is
+ * read has been written by the same call first. */
+#define CATAPULT_ESTIMATE_STATIC_MAX_N 2097152LL
+catapult_status catapult_estimate_static(int32_t g_kind, int64_t n, const int32_t *d_status,
+                                         const double *d_tstop, const double *d_g_user, double *d_out,
+                                         void *stream);
+
 /* launch geometry the tracer uses on the current device: persistent blocks and threads per block */
 catapult_status catapult_trace_launch_shape(const catapult_field *f, const catapult_trace_params *p,
                                             int32_t *blocks, int32_t *threads);

@@ -28,7 +28,7 @@ EXPORTS = [
     "catapult_field_table_bytes", "catapult_field_eval", "catapult_field_export_rows",
     "catapult_trace", "catapult_trace_init", "catapult_trace_continue", "catapult_trace_host",
     "catapult_trace_continue_host", "catapult_release_host_cache", "catapult_trace_scripted",
-    "catapult_step_once", "catapult_estimate", "catapult_trace_launch_shape", "catapult_last_error",
+    "catapult_step_once", "catapult_estimate", "catapult_estimate_static", "catapult_trace_launch_shape", "catapult_last_error",
     "catapult_version",
 ]
 PROBE_EXPORTS = ["catapult_math_probe", "catapult_measure_fp64_peak", "catapult_measure_l2_bandwidth",
@@ -88,6 +88,7 @@ def load():
     L.catapult_trace_scripted.argtypes = [vp, C.POINTER(TraceParams), i64, dp, C.c_int32, dp, dp, dp, dp, dp, vp]
     L.catapult_step_once.argtypes = [vp, C.POINTER(TraceParams), i64, dp, dp, dp, dp, dp, dp, vp]
     L.catapult_estimate.argtypes = [C.c_int32, i64, dp, dp, dp, dp, dp, vp]
+    L.catapult_estimate_static.argtypes = [C.c_int32, i64, dp, dp, dp, dp, vp]
     L.catapult_release_host_cache.argtypes = []
     L.catapult_trace_launch_shape.argtypes = [vp, C.POINTER(TraceParams), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     L.catapult_last_error.restype = C.c_char_p
@@ -378,6 +379,30 @@ def catapult_estimate(g_kind: int, d_status=None, d_tstop=None, d_g_user=None, t
     _check(load().catapult_estimate(g_kind, n, _ptr(d_status, torch.int32, True), _ptr(d_tstop, torch.float64, True),
                                     _ptr(d_g_user, torch.float64, True), _ptr(out), _hptr(h, np.float64), _stream()))
     return h if to_host else out
+
+
+ESTIMATE_STATIC_MAX_N = 2097152
+
+
+def catapult_estimate_static(g_kind: int, d_status=None, d_tstop=None, d_g_user=None, out=None):
+    """catapult_estimate for callers that must not allocate device memory (a process whose GPU memory is owned by its
+    own manager, a latency-bound loop, a driver without memory pools): same four numbers, bit-identical, with the
+    partial sums in a 16 KiB array built into the library instead of a stream-ordered allocation.
+
+    `out` is the caller's CUDA float64[4] result tensor, filled on the current stream and returned (nothing is copied
+    to the host).  Pass it: when it is omitted this wrapper makes one with torch.empty, which allocates -- fine in a
+    test, not what a no-allocation caller wants.  At most ESTIMATE_STATIC_MAX_N particles (CatapultError otherwise).
+    All calls on a GPU share the array: keep them on one stream or order them yourself.  The first call on a device
+    looks the array up; make it during set-up."""
+    torch = _torch()
+    ref = d_status if d_status is not None else (d_tstop if d_tstop is not None else d_g_user)
+    n = ref.shape[0]
+    if out is None:
+        out = torch.empty(4, dtype=torch.float64, device=ref.device)
+    _check(load().catapult_estimate_static(g_kind, n, _ptr(d_status, torch.int32, True),
+                                           _ptr(d_tstop, torch.float64, True), _ptr(d_g_user, torch.float64, True),
+                                           _ptr(out, torch.float64), _stream()))
+    return out
 
 
 FN_ATAN2, FN_SINCOS, FN_EXP, FN_SQRT_RSQRT, FN_RCP, FN_POW_NEG_INV, FN_CONTROLLER = range(7)

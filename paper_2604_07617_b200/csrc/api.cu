@@ -586,6 +586,18 @@ catapult_status catapult_estimate(int32_t g_kind, int64_t n, const int32_t* d_st
   return CATAPULT_OK;
 }
 
+// The estimate without any allocation (include/catapult.h): same validation as catapult_estimate, the size limit and
+// the static scratch array are estimate.cu's.
+catapult_status catapult_estimate_static(int32_t g_kind, int64_t n, const int32_t* d_status, const double* d_tstop,
+                                         const double* d_g_user, double* d_out, void* stream) {
+  if (n < 0) return fail(CATAPULT_EINVAL, "n < 0");
+  if (g_kind < 0 || g_kind > 2) return fail(CATAPULT_EINVAL, "g_kind must be 0, 1 or 2");
+  if (!d_out) return fail(CATAPULT_EINVAL, "d_out is NULL");
+  if (n > 0 && ((g_kind == 0 && !d_status) || (g_kind == 1 && !d_tstop) || (g_kind == 2 && !d_g_user)))
+    return fail(CATAPULT_EINVAL, "the array selected by g_kind is NULL");
+  return launch_estimate_static(g_kind, n, d_status, d_tstop, d_g_user, d_out, (cudaStream_t)stream);
+}
+
 catapult_status catapult_trace_launch_shape(const catapult_field* f, const catapult_trace_params* p, int32_t* blocks,
                                             int32_t* threads) {
   if (!blocks || !threads) return fail(CATAPULT_EINVAL, "blocks/threads is NULL");

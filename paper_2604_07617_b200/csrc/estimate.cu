@@ -75,4 +75,66 @@ catapult_status launch_estimate(int g_kind, int64_t n, const int* d_status, cons
   return CATAPULT_OK;
 }
 
+// ---- catapult_estimate_static: the same estimate for callers that are not allowed to allocate ---------------------
+// (include/catapult.h has the user-facing contract).  The per-block partial sums, which launch_estimate() above keeps
+// in a stream-ordered allocation, live here in an array that is part of the loaded library image: 16 KiB on every
+// GPU that loads libcatapult.so, held until the process exits, shared by every call on that GPU.
+//
+// Two things about this array are easy to get wrong:
+//  * In HOST code the name `estimate_static_scratch` is only a handle for the runtime, not a device address; handing
+//    it to a kernel makes the kernel fault (or scribble over host memory on systems where the GPU can reach it).
+//    The device address has to be asked for with cudaGetSymbolAddress, with the device in question current, and it is
+//    different on every device.  estimate_static_scratch_ptr() below does that once per device and remembers it.
+//  * Nothing here must start at zero: estimate_partial_kernel writes every slot [0, 2*blocks) that
+//    estimate_final_kernel reads, so whatever an earlier call left behind is never seen.
+constexpr int EST_STATIC_MAX_DEVICES = 64;
+static __device__ __align__(256) double estimate_static_scratch[2 * EST_MAX_BLOCKS];
+
+static_assert(CATAPULT_ESTIMATE_STATIC_MAX_N == (long long)EST_MAX_BLOCKS * EST_THREADS * 8,
+              "catapult.h's limit = one scratch slot per block of EST_THREADS * 8 particles");
+
+// Device address of the scratch array on the CURRENT device; looked up on the first call per device (no allocation:
+// cudaGetSymbolAddress only reports where the already loaded image put the array), cached afterwards.
+static catapult_status estimate_static_scratch_ptr(double** out) {
+  static double* cache[EST_STATIC_MAX_DEVICES] = {};  // written once per device; a racing duplicate writes the same value
+  int dev = -1;
+  CATAPULT_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev >= 0 && dev < EST_STATIC_MAX_DEVICES) {
+    double* c = __atomic_load_n(&cache[dev], __ATOMIC_ACQUIRE);
+    if (c) {
+      *out = c;
+      return CATAPULT_OK;
+    }
+  }
+  double* p = nullptr;
+  CATAPULT_CUDA_TRY(cudaGetSymbolAddress((void**)&p, estimate_static_scratch));
+  if (!p) {
+    set_error("cudaGetSymbolAddress(estimate_static_scratch) returned a null address");
+    return CATAPULT_ECUDA;
+  }
+  if (dev >= 0 && dev < EST_STATIC_MAX_DEVICES) __atomic_store_n(&cache[dev], p, __ATOMIC_RELEASE);
+  *out = p;
+  return CATAPULT_OK;
+}
+
+catapult_status launch_estimate_static(int g_kind, int64_t n, const int* d_status, const double* d_tstop,
+                                       const double* d_g, double* d_out, cudaStream_t s) {
+  if (n > CATAPULT_ESTIMATE_STATIC_MAX_N) {
+    set_error("catapult_estimate_static: n exceeds CATAPULT_ESTIMATE_STATIC_MAX_N (2097152 particles, the size its "
+              "built-in scratch array was made for); use catapult_estimate, which allocates its scratch");
+    return CATAPULT_EINVAL;
+  }
+  // the block partition of launch_estimate() for the same n (never capped below the limit above), so both entry
+  // points add the same numbers in the same order
+  const long long want = (n + EST_THREADS * 8 - 1) / (EST_THREADS * 8);
+  const int blocks = (int)(want < 1 ? 1 : want);
+  double* partial = nullptr;
+  catapult_status st = estimate_static_scratch_ptr(&partial);
+  if (st != CATAPULT_OK) return st;
+  estimate_partial_kernel<<<blocks, EST_THREADS, 0, s>>>(g_kind, n, d_status, d_tstop, d_g, partial);
+  estimate_final_kernel<<<1, 32, 0, s>>>(n, blocks, partial, d_out);
+  CATAPULT_CUDA_TRY(cudaGetLastError());
+  return CATAPULT_OK;
+}
+
 }  // namespace catapult

@@ -81,6 +81,9 @@ catapult_status trace_launch_shape(int model, int64_t n, int* blocks, int* threa
 // estimate.cu
 catapult_status launch_estimate(int g_kind, int64_t n, const int* d_status, const double* d_tstop,
                                 const double* d_g, double* d_out, cudaStream_t s);
+// same sums, partial results in the library's own static device array: no allocation (catapult_estimate_static)
+catapult_status launch_estimate_static(int g_kind, int64_t n, const int* d_status, const double* d_tstop,
+                                       const double* d_g, double* d_out, cudaStream_t s);
 
 // mathprobe.cu
 catapult_status launch_math_probe(int fn, int64_t n, const double* d_a, const double* d_b, double* d_o0, double* d_o1,

@@ -17,9 +17,13 @@
  *   - Calls validate their arguments synchronously, enqueue work on `stream` and do not
  *     synchronise (device memory they need is allocated and freed stream-ordered), except: the
  *     *_host variants and catapult_estimate with a non-NULL h_out, which return after their
- *     results are in host memory, and catapult_field_destroy / catapult_release_host_cache,
- *     which free device memory (cudaFree).  A field may be used on any stream: every call that
- *     reads its tables is ordered after the build by an event the build recorded.
+ *     results are in host memory, catapult_field_destroy, which waits for ALL work on the field's
+ *     device (cudaDeviceSynchronize: traces of the field may be running on any stream) before it
+ *     frees the tables, so a field may be destroyed right after an asynchronous call that uses it,
+ *     and catapult_release_host_cache (cudaFree of the calling thread's staging slab, which came
+ *     from cudaMalloc and therefore waits for the device).
+ *     A field may be used on any stream: every call that reads its tables is ordered after the
+ *     build by an event the build recorded.
  *   - There is no CPU fallback anywhere: without a CUDA device every compute call fails with
  *     CATAPULT_ECUDA.
  *   - Particle arrays are structure-of-arrays: x[4][n] means component c of particle i at
@@ -40,7 +44,7 @@ typedef enum {
   CATAPULT_EINVAL = 1,       /* bad argument (NULL required pointer, n<0, ncell<1, non-finite T/rtol/atol ...) */
   CATAPULT_ENOMEM = 2,       /* device or host allocation failed */
   CATAPULT_ECUDA = 3,        /* CUDA runtime error (message in catapult_last_error) */
-  CATAPULT_EUNSUPPORTED = 4  /* valid but not built (e.g. non-vacuum Boozer I != 0) */
+  CATAPULT_EUNSUPPORTED = 4  /* valid but not built (e.g. a non-canonical column order, the wave on a non-vacuum field) */
 } catapult_status;
 
 #define CATAPULT_COORD_BOOZER 0 /* grid (s,theta,zeta); particles (s,theta,zeta,vpar)            */
@@ -53,7 +57,8 @@ typedef enum {
 #define CATAPULT_NQUANT_BOOZER 4
 /* Boozer, derivative-of-interpolant mode (R1c): only |B| is tabulated (nquant = 1, one 512-byte block per
    cell instead of four); d|B|/ds, d|B|/dtheta, d|B|/dzeta are the derivatives of its local tricubic.  The right-hand
-   side then jumps at cell faces: more and more often rejected steps than with tabulated derivative columns. */
+   side then jumps at cell faces: more attempts are rejected and more steps are needed than with tabulated
+   derivative columns. */
 #define CATAPULT_NQUANT_BOOZER_DOI 1
 #define CATAPULT_NQUANT_CYL 7
 
@@ -133,8 +138,11 @@ typedef struct {
  * order).  One cell's coefficients of one quantity are four 128-byte lines.
  * catapult_field_export_rows recovers the nodal values in the paper's own row layout.  *out owns the
  * table (allocated stream-ordered on `stream`); d_nodes may be freed once the stream has run.
- * Errors: EINVAL (NULL, ncell<1 or more than 2^31-1 cells, nquant mismatch, hi<=lo), EUNSUPPORTED
- * (Boozer I0 != 0, tabulated profiles, non-canonical column order), ENOMEM, ECUDA. */
+ * Errors: EINVAL (NULL, ncell<1 or more than 2^31-1 cells, nquant mismatch, hi<=lo, nfp<1, G0 == 0 for a
+ * Boozer field -- also when profiles are given: G0 then only has to be non-zero, G(s) comes from G_nodes --,
+ * only some of the three profile pointers), EUNSUPPORTED (a constant I0 != 0 without profiles: give I(s) as a
+ * profile instead; non-canonical column order), ENOMEM, ECUDA.  When the build fails after the table was
+ * allocated, the call waits for `stream` before it frees the table. */
 catapult_status catapult_field_build(const catapult_field_desc *desc, const double *d_nodes,
                                      void *stream, catapult_field **out);
 /* same with HOST nodes: copies them to the device, builds, synchronises, frees the staging copy */
@@ -183,8 +191,10 @@ catapult_status catapult_trace_continue(const catapult_field *f, const catapult_
 /* HOST-buffer form of catapult_trace: copies h_x0 to the device, traces, copies the results back
    and synchronises.  h_nacc/h_nrej/h_counters may be NULL.  The *_host calls keep one device staging
    slab and one non-blocking stream per host thread between calls (grown on demand);
-   catapult_release_host_cache frees the calling thread's.  Pinned host buffers make the copies
-   asynchronous with respect to the host. */
+   catapult_release_host_cache frees the calling thread's.  Nothing frees them at thread exit (the CUDA
+   context may already be gone by then): a thread that used a *_host call and ends without calling
+   catapult_release_host_cache leaves its slab and stream allocated until the process ends.  Pinned host
+   buffers make the copies asynchronous with respect to the host. */
 catapult_status catapult_trace_host(const catapult_field *f, const catapult_trace_params *p,
                                     int64_t n, const double *h_x0, double *h_xf, double *h_tstop,
                                     int32_t *h_status, uint32_t *h_nacc, uint32_t *h_nrej,

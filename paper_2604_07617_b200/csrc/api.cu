@@ -229,6 +229,9 @@ catapult_status catapult_field_build(const catapult_field_desc* desc, const doub
     if (e != cudaSuccess) st = cuda_fail(e, "cudaEventRecord(built)");
   }
   if (st != CATAPULT_OK) {
+    // the table came from cudaMallocAsync: cudaFree does not wait for work that still uses it, and the build kernel or
+    // the profile copies may be in flight on `stream`
+    cudaStreamSynchronize((cudaStream_t)stream);
     if (f->built) cudaEventDestroy(f->built);
     cudaFree(f->d_table);
     delete f;
@@ -266,9 +269,20 @@ catapult_status catapult_field_build_host(const catapult_field_desc* desc, const
 
 catapult_status catapult_field_destroy(catapult_field* f) {
   if (!f) return CATAPULT_OK;
+  // The table is a stream-ordered allocation, and for those cudaFree returns the memory WITHOUT waiting for kernels
+  // that still read it (unlike memory from cudaMalloc).  Traces and evaluations of this field may be running on any
+  // stream of its device, so the whole device is drained first; otherwise `del field` right after an asynchronous
+  // trace would hand the table to the next allocation under the running tracer.
+  int cur = -1;
+  cudaError_t e = cudaGetDevice(&cur);
+  if (e == cudaSuccess && cur != f->device) e = cudaSetDevice(f->device);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
   if (f->built) cudaEventDestroy(f->built);
   if (f->d_table) cudaFree(f->d_table);
+  if (cur >= 0 && cur != f->device) cudaSetDevice(cur);
   delete f;
+  // an error left behind by earlier asynchronous work is reported, but the field is gone either way
+  if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceSynchronize before freeing the field's table");
   return CATAPULT_OK;
 }
 

@@ -746,6 +746,12 @@ trace_pair_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__
             for (int c = 0; c < 4; ++c) a.kall[((long long)j * 4 + c) * n + idx] = j < 6 ? ks[(j * 4 + c) * NS] : dy[c];
           active = false;
           report = REPORT_NO_STATUS;
+          if (!(chk == chk) || fabs(chk) > 1.7e308) {
+            // same guard as above, after the derivatives have been reported: the next particle in this slot must
+            // not meet 0 * NaN in its stage sums
+#pragma unroll 1
+            for (int j = 4; j < 24; ++j) ks[j * NS] = 0.0;
+          }
         }
         if (MODE != MODE_STEP_ONCE) {
           if (!accepted) {

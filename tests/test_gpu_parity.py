@@ -173,6 +173,71 @@ def test_single_step_parity(K, oracle, cases, idx):
     print(f"cfg{idx}: single step, worst relative difference of the error ratio {worst_r:.2e}")
 
 
+def test_step_once_poisoned_particle_does_not_spoil_its_slot(K, oracle, cases):
+    """One attempted step per particle on more particles than the launch has slots, so that slots are reused.  A few
+    particles are given a step length that makes every derivative non-finite (NaN / Inf h).  Every OTHER particle must
+    return exactly what it returns without the poisoned ones in the batch (the stage sums multiply zero tableau
+    entries with whatever derivative the slot's previous particle left: 0 * NaN would leak), the poisoned ones must
+    report non-finite results, and a sample of the clean ones is compared with the oracle at the single-step bar."""
+    c = cases[2]
+    cfg = W.config(2, n=60_000, T=1e-5, ncell=SMALL[2]["ncell"], with_nodes=False)
+    blocks, threads = K.catapult_trace_launch_shape(c["gf"], cfg["params"])
+    x0 = cfg["x0"]
+    n = x0.shape[1]
+    assert n > blocks * threads, "the batch must be larger than the number of slots of the launch"
+    rng = np.random.default_rng(31)
+    t = 1e-6 * rng.random(n)
+    h = cfg["params"]["dtmax"] * (0.02 + 0.1 * rng.random(n))
+    clean = K.catapult_step_once(c["gf"], cfg["params"], _dev(x0), _dev(t), _dev(h))
+    clean = [v.cpu().numpy() for v in clean]
+    assert all(np.isfinite(v).all() for v in clean)
+    hp = h.copy()
+    poison = rng.choice(n // 2, size=400, replace=False)          # in the first half: their slots are refilled later
+    hp[poison[::2]] = np.nan
+    hp[poison[1::2]] = np.inf
+    got = [v.cpu().numpy() for v in K.catapult_step_once(c["gf"], cfg["params"], _dev(x0), _dev(t), _dev(hp))]
+    ok = np.ones(n, dtype=bool)
+    ok[poison] = False
+    assert np.array_equal(got[0][:, ok], clean[0][:, ok])
+    assert np.array_equal(got[1][ok], clean[1][ok])
+    assert np.array_equal(got[2][:, :, ok], clean[2][:, :, ok])
+    assert not np.isfinite(got[1][poison]).any() and not np.isfinite(got[0][:, poison]).all(axis=0).any()
+    sc = _state_scale(0)
+    for i in rng.choice(np.flatnonzero(ok), size=64, replace=False):
+        xo, ro, ko = oracle.step_once(c["of"], c["op"], x0[:, i], t[i], h[i])
+        assert np.all(np.abs(_stepped(0, got[0][:, i]) - _stepped(0, xo)) <= 1e-11 * sc), i
+        assert np.all(np.abs(got[2][:, :, i] - ko) <= 1e-11 * np.abs(ko).max(axis=0)[None, :] + 1e-300), i
+
+
+def test_field_destroyed_right_after_an_unsynchronised_trace(K, cases):
+    """`f = build(...); out = trace(f, ...); del f` without any synchronisation in between, on a side stream.  The
+    table is a stream-ordered allocation, for which cudaFree does not wait by itself: catapult_field_destroy has to
+    drain the device first (include/catapult.h), otherwise the allocations that follow here would reuse the table
+    under the running tracer.  The result must equal the one of a run that synchronises before the field goes."""
+    cfg = W.config(2, n=30_000, T=2e-5, ncell=SMALL[2]["ncell"])
+    x0 = _dev(cfg["x0"])
+    gf = K.catapult_field_build(cfg["field"])
+    want = K.catapult_trace(gf, cfg["params"], x0)
+    torch.cuda.synchronize()
+    want = {k: want[k].cpu().numpy() for k in ("xf", "tstop", "status", "nacc")}
+    gf.destroy()
+    poisoned = dict(cfg["field"], nodes=np.full_like(cfg["field"]["nodes"], np.nan))
+    side = torch.cuda.Stream()
+    for _ in range(3):
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            gf = K.catapult_field_build(cfg["field"])
+            got = K.catapult_trace(gf, cfg["params"], x0)        # asynchronous: the kernel is still running ...
+            gf.destroy()                                          # ... when the field is destroyed
+            # what a careless free would let happen: the next stream-ordered allocation of the same size takes the
+            # table's memory and a build kernel fills it with other numbers
+            other = K.catapult_field_build(poisoned)
+            other.destroy()
+        side.synchronize()
+        for k, v in want.items():
+            assert np.array_equal(got[k].cpu().numpy(), v), k
+
+
 # ---- whole trajectories over the 1e-5 s window ----------------------------------------------------
 def _stepped(coord, x):
     """API state -> the variables the tracer steps and Eq. 4 scores: (s cos th, s sin th, zeta, vpar)."""

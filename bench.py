@@ -14,11 +14,12 @@ WINDOW LEG (the timed K steps; `value`).  One "step" = one pass of the whole hot
 estimate (a10).  Consecutive steps trace consecutive windows [j*w, (j+1)*w] of the same job with the state carried
 on the device (catapult_trace_continue).  The metric (accepted DP5 steps per second) is intensive.
 
-JOB LEG (`full_job`, the second half of BASELINE.json's metric: particles-to-T per second).  The first
-`--job-particles` particles of the same ensemble traced from t = 0 to the config's own T (1e-2 s) in ONE
-catapult_trace launch: the population thins as particles are lost and the tail runs under-filled, so the job-level
-rate is what a user sees.  `--job-particles -1` traces the full ensemble (cfg4: ~10 GPU-minutes; the lines of those
-runs are committed under profiles/).
+JOB LEG (`full_job`, the second half of BASELINE.json's metric: particles-to-T per second).  The ensemble traced from
+t = 0 to the config's own T (1e-2 s) in ONE catapult_trace launch: the population thins as particles are lost and
+the tail runs under-filled, so the job-level rate is what a user sees.  The default (`--job-particles -1`) is the
+WHOLE ensemble, the config the metric is quoted on (cfg4: 10^6 particles, ~10 GPU-minutes, which dominates the run
+time of the default command); `--job-particles 65536` is the quick form (slot efficiency 0.83 instead of 0.98, so
+its particles-to-T/s is ~15 % lower), `--job-particles 0` skips the leg.
 
 N > 1: ONE seeded ensemble of N x particles, split over the ranks by interleaved index, tables
 replicated, no data-path collective; one 24-byte all-reduce of (sum g, sum g^2, n) gives the estimate.  Per-GPU work
@@ -65,6 +66,13 @@ ALG_FLOPS_PER_ATTEMPT = 150
 # evaluation, lanes without a particle included).  `roofline.executed` uses these; stage algebra included.
 EXEC_FLOPS_PER_EVAL = {"boozer_vac": 4 * 126 + 275, "boozer_saw": 4 * 126 + 375, "cart": 7 * 126 + 260}
 EXEC_FLOPS_PER_EVAL.update({"boozer_vac_doi": 224 + 290, "boozer_saw_doi": 224 + 390})
+# The part of the executed work that is known EXACTLY, without any capture: the contraction's 63 FMA per quantity
+# (m quantities; derivative-of-interpolant mode: 112 FMA for value and gradient).  `roofline.contraction_only` uses
+# these and leaves the scalar side out: a lower bound of the executed rate that no hand-entered constant enters.
+# (`roofline.frac` stays the ALGORITHMIC figure: that is the bench contract's definition of `achieved`, SURVEY 8(d);
+# the scalar-side constants of EXEC_FLOPS_PER_EVAL come from ONE capture of cfg4 and are not re-derived per build.)
+CONTRACTION_FLOPS_PER_EVAL = {"boozer_vac": 4 * 126, "boozer_saw": 4 * 126, "cart": 7 * 126, "boozer_vac_doi": 224,
+                              "boozer_saw_doi": 224}
 # particle slots served by one thread block (tracer_pair.cu: two warp pairs; tracer.cu: one scalar warp)
 SLOTS_PER_BLOCK = {"boozer_vac": 64, "boozer_saw": 64, "cart": 32, "boozer_vac_doi": 64, "boozer_saw_doi": 64}
 BYTES_PER_CELL_VISIT = {"boozer_vac": 4 * 512, "boozer_saw": 4 * 512, "cart": 7 * 512, "boozer_vac_doi": 512, "boozer_saw_doi": 512}
@@ -230,14 +238,16 @@ def main():
                     "take its derivatives from the interpolant (DESIGN.md R1c, SURVEY 8(f) f2): a quarter of the table")
     ap.add_argument("--rtol", type=float, default=0.0, help="tracing tolerance (0 = the config's 1e-9): PAPER.md:100-102")
     ap.add_argument("--e2e-steps", type=int, default=-1, help="steps of the host-buffer leg (-1 = --steps, 0 = skip)")
-    ap.add_argument("--job-particles", type=int, default=65536,
-                    help="particles of the full-T job leg (0 = skip, -1 = the whole ensemble)")
+    ap.add_argument("--job-particles", type=int, default=-1,
+                    help="particles of the full-T job leg (-1 = the whole ensemble, the config BASELINE.json's metric is "
+                         "quoted on: ~10 min for cfg4's 10^6 particles; 65536 = a quick run; 0 = skip)")
     ap.add_argument("--job-T", type=float, default=0.0, help="end time of the job leg (0 = the config's own T)")
     ap.add_argument("--job-oracle", type=int, default=0, help="fidelity leg of the sweep (PAPER.md:98-102): the oracle traces "
                     "the first N particles of the job leg to the same end time; loss fractions and per-particle loss "
                     "flags are compared (0 = skip)")
     ap.add_argument("--cpu-particles", type=int, default=2048, help="oracle sample for cpu_baseline (0 = skip)")
-    ap.add_argument("--ref-particles", type=int, default=1024)
+    ap.add_argument("--ref-particles", type=int, default=2048, help="oracle sample of --impl reference: the same sample "
+                    "as the cpu_baseline leg of the GPU arm (first N particles, [0, window])")
     ap.add_argument("--no-peaks", action="store_true")
     ap.add_argument("--dry-run-ranks", action="store_true", help="every rank prints its environment and exits")
     args = ap.parse_args()
@@ -373,7 +383,13 @@ def main():
                 "nominal 148 SM x 64 DFMA/clk x 1.965 GHz",
                 "flops_per_rhs_eval": ALG_FLOPS_PER_EVAL[model], "flops_per_attempt": ALG_FLOPS_PER_ATTEMPT,
                 "executed": {"achieved": exe, "frac": exe / peak, "flops_per_rhs_eval": EXEC_FLOPS_PER_EVAL[model],
-                             "note": "the kernel's own arithmetic (63-FMA Horner per quantity, no Lagrange basis)"},
+                             "note": "the kernel's own arithmetic (63-FMA Horner per quantity, no Lagrange basis); the "
+                                     "scalar-side constant is from one ncu capture of cfg4 (profiles/r2_ncu_trace_pair.md)"},
+                "contraction_only": {"achieved": cnt[6] * CONTRACTION_FLOPS_PER_EVAL[model] / trace_s / 1e12,
+                                     "frac": cnt[6] * CONTRACTION_FLOPS_PER_EVAL[model] / trace_s / 1e12 / peak,
+                                     "flops_per_rhs_eval": CONTRACTION_FLOPS_PER_EVAL[model],
+                                     "note": "exactly known flops of the tricubic contraction alone; locate, right-hand "
+                                             "side and stage algebra excluded"},
                 "traffic": dram_b * evals_per_launch if dram_b else None,
                 "traffic_source": "profiles/r2_traffic_pair.csv (committed ncu --set full capture, bytes per evaluation) "
                                   "x the evaluations of one timed launch" if dram_b else None,

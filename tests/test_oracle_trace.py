@@ -365,3 +365,60 @@ def test_derivative_of_interpolant_mode(oracle):
     assert r1["nacc"].sum() > 1.2 * r4["nacc"].sum()          # more steps ...
     rej = lambda r: r["nrej"].sum() / (r["nacc"].sum() + r["nrej"].sum())
     assert rej(r1) > rej(r4)                                  # ... and more of the attempts rejected
+
+
+def _psi_closed_form(x):
+    """Config 3's level function in closed form (workloads.cyl_field_values): psi = B0/(2 q0) [(R-R0)^2 + (Z/kappa)^2].
+    It is a quadratic in (R, Z), so its local tricubic reproduces it to rounding: the interpolated level the tracer
+    tests and this expression agree to ~1e-15 psi_edge, and the loss surface is the ellipse
+    (R-R0)^2 + (Z/kappa)^2 = a^2."""
+    R = np.hypot(x[0], x[1])
+    return (W.B0 / (2.0 * W.Q0_CYL)) * ((R - W.R0) ** 2 + (x[2] / W.KAPPA_CYL) ** 2)
+
+
+def test_cartesian_loss_is_the_first_accepted_state_beyond_the_closed_form_surface(oracle):
+    """"in Cartesian coordinates we detect a sign change in the interpolation of a signed distance
+    function" -- here the level function psi - psi_edge in column 6 (R3).  Pins of orc_is_lost's
+    cylindrical branch against the closed-form surface, none of which uses the oracle's own interpolation:
+    born outside => status 1, t_stop 0, state unchanged, no step; born just inside => steps are taken; along every
+    recorded trajectory the status flips exactly at the first accepted end state with psi >= psi_edge (all earlier
+    states are inside, the last one of a lost particle is outside, particles that reach T never were outside)."""
+    O = oracle
+    cfg = W.config(3, n=4, T=2e-5, ncell=[12, 11, 5])
+    f, p = O.Field(cfg["field"]), O.make_params(cfg["params"])
+    edge = W.PSI_EDGE_CYL
+    # interpolated level == closed form on and around the surface (cubic exactness), so the pin below has teeth
+    rng = np.random.default_rng(11)
+    xs = W.cyl_births(rng, 32, psi_frac=1.0)
+    R, phi = np.hypot(xs[0], xs[1]), np.mod(np.arctan2(xs[1], xs[0]), 2 * np.pi)
+    lev = O.tricubic_many(f, np.array([R, xs[2], phi]))[6]
+    assert np.max(np.abs(lev - _psi_closed_form(xs))) < 1e-13 * edge
+    # born outside / just inside
+    out = W.cyl_births(np.random.default_rng(12), 8, psi_frac=1.1)
+    r = O.trace(f, p, out)
+    assert np.all(r["status"] == 1) and np.all(r["tstop"] == 0.0) and np.array_equal(r["xf"], out)
+    assert np.all(r["nacc"] == 0) and np.all(r["nrej"] == 0)
+    inside = W.cyl_births(np.random.default_rng(12), 8, psi_frac=1.0 - 1e-6)
+    r = O.trace(f, p, inside)
+    assert np.all(r["tstop"] > 0.0) and np.all(r["nacc"] >= 1)
+    # crossing: births on 0.97 psi_edge, many leave within the window
+    x0 = W.cyl_births(np.random.default_rng(13), 64, psi_frac=0.97)
+    r = O.trace(f, p, x0)
+    nlost = int(np.sum(r["status"] == 1))
+    assert 10 <= nlost <= 60, nlost                      # both outcomes are present
+    margin = 1e-12 * edge
+    for i in range(x0.shape[1]):
+        traj, ts, st = O.trace_record(f, p, x0[:, i])
+        assert st == r["status"][i] and ts == r["tstop"][i]
+        psi = _psi_closed_form(traj[:, 1:5].T)
+        assert np.all(np.abs(psi - edge) > margin)       # no state so close that rounding decides
+        assert np.all(psi[:-1] < edge), i                # every state before the last is inside ...
+        if st == 1:
+            assert psi[-1] >= edge and traj[-1, 0] == ts and ts < 2e-5, i    # ... and a lost one ends outside
+            assert np.array_equal(traj[-1, 1:5], r["xf"][:, i])
+        else:
+            assert st == 0 and psi[-1] < edge and ts == 2e-5, i
+    # a wrong level column, or the Boozer flux psi0 in place of psi_edge, changes the verdicts: the closed form on the
+    # final states alone separates the two classes
+    pf = _psi_closed_form(r["xf"])
+    assert np.array_equal(pf >= edge, r["status"] == 1)

@@ -974,7 +974,7 @@ def test_derivative_of_interpolant_single_step_parity(K, oracle, doi_cases, name
     assert c["gf"].table_bytes * 4 == K.catapult_field_build(cfg["field"]).table_bytes
 
 
-@pytest.mark.parametrize("name", ["vac", "saw"])
+@pytest.mark.parametrize("name", ["vac", "saw", "nv"])
 def test_derivative_of_interpolant_trajectory_parity(K, oracle, doi_cases, name):
     """Scripted replay over 1e-5 s and the free-running adaptive run (statuses, accepted-step total).  The trajectory bar
     is 1e-6 here, 100x the four-table mode's 1e-8: every evaluation's derivatives agree 100-300x less well (round-off
@@ -1179,3 +1179,53 @@ def test_energy_drift_on_the_refined_grid(K, oracle):
     do = np.abs((0.5 * o["xf"][3] ** 2 + mu[:8] * Bo) / (0.5 * W.V_TOTAL ** 2) - 1)
     assert do[ko].max() <= 1e-6
     gf.destroy()
+
+
+@pytest.mark.parametrize("which", ["nv", "doi_vac", "doi_saw", "doi_nv"])
+def test_loss_time_inside_the_step_on_the_other_boozer_variants(K, oracle, nonvacuum_case, doi_cases, which):
+    """loss_time_mode 1 (DESIGN.md S5b) is one piece of code serving every Boozer variant of the warp-pair tracer;
+    test_loss_time_inside_the_step covers the four-column vacuum and wave models.  Here: tabulated profiles, and the
+    derivative-of-interpolant mode with each of the three right-hand sides.  Scripted replay of the oracle's step
+    sequence: stop time (as a fraction of the crossing step, times the step's radial displacement) and state to the
+    variant's own trajectory bar (1e-8 with tabulated
+    derivative columns, 1e-6 in derivative-of-interpolant mode), every lost particle ends ON the boundary."""
+    c = nonvacuum_case if which == "nv" else doi_cases[which[4:]]
+    bar = 1e-8 if which == "nv" else 1e-6
+    cfg = c["cfg"]
+    x0 = cfg["x0"].copy()
+    n = x0.shape[1]
+    x0[0, ::3] = 0.992 + 0.007 * np.linspace(0.0, 1.0, len(x0[0, ::3]))
+    p0 = dict(cfg["params"], T=2e-5)
+    p1 = dict(p0, loss_time_mode=1)
+    op0, op1 = oracle.make_params(p0), oracle.make_params(p1)
+    recs = [oracle.trace_record(c["of"], op0, x0[:, i]) for i in range(n)]
+    hs = [np.diff(r[0][:, 0]) for r in recs]
+    H = np.zeros((max(len(h) for h in hs) + 1, n))
+    for i, h in enumerate(hs):
+        H[:len(h), i] = h
+    g = K.catapult_trace_scripted(c["gf"], p1, _dev(x0), _dev(H))
+    gx, gt, gs = (g[k].cpu().numpy() for k in ("xf", "tstop", "status"))
+    sc = _state_scale(0)
+    nlost, worst, worst_t = 0, 0.0, 0.0
+    for i in range(n):
+        xo, to, so, _ = oracle.trace_scripted(c["of"], op1, x0[:, i], hs[i])
+        assert gs[i] == so
+        if so != 1:
+            assert gt[i] == to
+            continue
+        nlost += 1
+        hlast = hs[i][-1]
+        assert recs[i][1] - hlast < to <= recs[i][1]                    # inside the crossing step
+        # The root theta* of s(theta) = 1 moves by (difference of the interpolated states) / (ds / dtheta): with the
+        # step's end states agreeing to `bar`, the loss time agrees to bar / |s_end - s_start| of the step length
+        # (a grazing crossing, small radial displacement, is the ill-conditioned case in any arithmetic).
+        ya, yb = recs[i][0][-2, 1:3], recs[i][0][-1, 1:3]
+        ds = abs(math.hypot(yb[0], yb[1]) - math.hypot(ya[0], ya[1]))
+        worst_t = max(worst_t, abs(gt[i] - to) / hlast * ds)
+        d = _state_diff(0, gx[:, i:i + 1], xo[:, None])[:, 0]
+        worst = max(worst, (np.abs(d) / np.maximum(sc, np.abs(xo))).max())
+        assert 1.0 <= gx[0, i] < 1.0 + 1e-9
+    print(f"{which}: {nlost} lost; loss time inside the step: worst difference x radial displacement {worst_t:.2e} "
+          f"of the step, state {worst:.2e}")
+    assert nlost >= 6
+    assert worst_t <= bar and worst <= bar

@@ -620,7 +620,7 @@ catapult_status catapult_trace_launch_shape(const catapult_field* f, const catap
   catapult_status st = make_trace_const(f, p, &tc, &model);
   if (st != CATAPULT_OK) return st;
   int b = 0, t = 0;
-  st = trace_launch_shape(model, (int64_t)1 << 40, &b, &t);
+  st = trace_launch_shape(model, f->fc.m == 1 && f->fc.coord == CATAPULT_COORD_BOOZER, (int64_t)1 << 40, &b, &t);
   *blocks = b;
   *threads = t;
   return st;

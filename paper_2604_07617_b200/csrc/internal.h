@@ -76,7 +76,7 @@ catapult_status launch_field_export_rows(const FieldConst& fc, int64_t ncells, d
 
 // tracer.cu (mode: 0 adaptive, 1 scripted replay, 2 one attempted step)
 catapult_status launch_trace(const TraceConst& tc, const TraceArgs& a, int model, int mode, cudaStream_t s);
-catapult_status trace_launch_shape(int model, int64_t n, int* blocks, int* threads);
+catapult_status trace_launch_shape(int model, bool doi, int64_t n, int* blocks, int* threads);
 
 // estimate.cu
 catapult_status launch_estimate(int g_kind, int64_t n, const int* d_status, const double* d_tstop,

@@ -32,6 +32,9 @@ namespace catapult {
 
 template <int MODEL>
 struct TraceTraits {
+  // this file serves the cylindrical model only (launch_trace below); the Boozer models, the wave included, are
+  // tracer_pair.cu's.  The MODEL parameter stays because eval_physics / is_lost / AxisRoles are shared templates.
+  static_assert(MODEL == MODEL_CART, "tracer.cu is instantiated for the cylindrical model only");
   static constexpr bool CART = (MODEL == MODEL_CART);
   static constexpr int NQ = CART ? CATAPULT_NQUANT_CYL : CATAPULT_NQUANT_BOOZER;
   static constexpr int NT = 32 * (NQ + 1);   // threads per block
@@ -271,23 +274,9 @@ __device__ __forceinline__ void scalar_round(const TraceConst& tc, unsigned char
   reqbuf[lane] = (act ? 1 : 0) | (kind << 1) | (sr.rpar << 6);
   __syncwarp();
   bar_arrive(BAR_A, NT);
-  // ---- in the shadow of the arctangent: unit vector, wave terms
+  // ---- in the shadow of the arctangent: the unit vector
   g.ca = (BZ && !(g.a > 0.0)) ? 1.0 : X[0] * g.inva;
   g.sa = X[1] * g.inva;
-  if (MODEL == MODEL_BOOZER_SAW) {
-    const double ds = g.a - tc.saw_s0;
-    g.Phihat = tc.saw_Phi0 * fm::exp(-ds * ds * tc.saw_invw2);
-    g.dPhihat = g.Phihat * (-2.0 * ds * tc.saw_invw2);
-    // sin / cos of m theta - n zeta + omega t by the addition theorem: cos / sin of theta are y0/s, y1/s, so the
-    // wave does not wait for the arctangent
-    const double beta = fma(-(double)tc.saw_n, X[2], tc.saw_omega * tr);
-    double sb, cb, cm, sm;
-    fm::sincos(beta, sb, cb);
-    unit_power(tc.saw_m, g.ca, g.sa, cm, sm);
-    g.sn = fma(sm, cb, cm * sb);
-    g.cs = fma(cm, cb, -sm * sb);
-    eval_wave_terms(tc, g);
-  }
   // ---- the last coordinate and the cell
   {
     const double ang = fm::atan2(X[1], X[0]);
@@ -713,8 +702,8 @@ catapult_status launch_trace(const TraceConst& tc, const TraceArgs& a, int model
   }
 }
 
-catapult_status trace_launch_shape(int model, int64_t n, int* blocks, int* threads) {
-  if (model != MODEL_CART) return trace_pair_shape(model, n, blocks, threads);
+catapult_status trace_launch_shape(int model, bool doi, int64_t n, int* blocks, int* threads) {
+  if (model != MODEL_CART) return trace_pair_shape(model, doi, n, blocks, threads);
   return trace_shape<MODEL_CART, MODE_ADAPTIVE>(n, blocks, threads);
 }
 

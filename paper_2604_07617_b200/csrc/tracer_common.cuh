@@ -246,6 +246,6 @@ __device__ __forceinline__ void eval_physics(const TraceConst& tc, const double 
 
 // tracer_pair.cu
 catapult_status launch_trace_pair(const TraceConst& tc, const TraceArgs& a, int model, int mode, cudaStream_t s);
-catapult_status trace_pair_shape(int model, int64_t n, int* blocks, int* threads);
+catapult_status trace_pair_shape(int model, bool doi, int64_t n, int* blocks, int* threads);
 
 }  // namespace catapult

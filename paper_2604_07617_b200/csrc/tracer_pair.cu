@@ -9,7 +9,7 @@
 //   * the SCALAR warp: lane l owns particle slot l -- state, DP5 stage states and sums, cell locate (square root,
 //     arctangent), the wave terms, the guiding-centre physics, error norm, controller, stop test and refill.
 //   * the CONTRACTION warp: lane l owns ALL 256 tricubic coefficients (4 quantities x 64, 2 KiB) of slot l's
-//     current cell on chip -- the first PAIR_NREG in registers, the others in a private conflict-free run of shared
+//     current cell on chip -- the first PairTraits::NREG in registers, the others in a private conflict-free run of shared
 //     memory -- re-fetched from the cell-major table only when the slot's cell changes: the register part by
 //     256-bit read-only loads straight into its final registers, the shared part by ONE bulk asynchronous copy
 //     (cp.async.bulk) signalled on a thread-private mbarrier.
@@ -33,17 +33,10 @@
 
 namespace catapult {
 
-#ifndef CATAPULT_PAIR_AHEAD
-#define CATAPULT_PAIR_AHEAD 1
-#endif
-#ifndef CATAPULT_PAIR_NREG
-#define CATAPULT_PAIR_NREG 88
-#endif
-
 struct PairTraits {
   static constexpr int NQ = CATAPULT_NQUANT_BOOZER;
   static constexpr int NCOEF = NQ * 64;
-  static constexpr int NREG = CATAPULT_PAIR_NREG;  // coefficients a contraction thread keeps in registers
+  static constexpr int NREG = 88;                   // coefficients a contraction thread keeps in registers
   static constexpr int NSH = NCOEF - NREG;         // ... and in shared memory
   static constexpr int NT = 128;                   // threads per block: two pairs of warps
   static constexpr int NS = 64;                    // particle slots per block
@@ -148,13 +141,25 @@ __device__ __forceinline__ void quad_rows(const double (&c)[4][4], double wF, do
   }
 }
 
+// Makes the calling thread wait HERE for the 256-bit loads that fill its coefficient registers, instead of at their
+// first use inside the contraction (which sits behind the REQ barrier, on the critical path of the round).  `last` is
+// the register the LAST issued load writes; loads of one thread to distinct registers return in order on this part,
+// so when it has landed all have.  The compiler cannot be told "wait for the scoreboard" directly: the only way is an
+// instruction that consumes the register, and it must not be removable.  Comparing the high word with a constant and
+// branching to a side effect does that.  The constant is the high word of a quiet NaN with an arbitrary payload; a
+// table never holds it unless the caller's nodes were NaN, and if one ever did, the only consequence is a sleep of
+// about a nanosecond: the test can cost time, it cannot change a result.
+__device__ __forceinline__ void wait_for_register_loads(double last) {
+  if (__double2hiint(last) == 0x7ffdead0) asm volatile("nanosleep.u32 1;");
+}
+
 // Plane values P[a][q] = sum_bc C[q][a][b][c] wS^b wF^c of the four quantities on the cell held: every row (c) by
 // Horner in wF, the four rows of a plane by Horner in wS from b = 3 down -- the operations and the order of
 // horner_plane (gc_device.cuh), which every user of the table follows.  The 64 rows are walked with the quantity
 // running fastest (quad_rows: 16 quads, plane a = 3 first); the rows of a quad that live in shared memory are
-// loaded PAIR_AHEAD quads ahead into rotating row buffers; a finished plane goes to the exchange buffer at once.
+// loaded PairRows::AHEAD quads ahead into rotating row buffers; a finished plane goes to the exchange buffer at once.
 struct PairRows {  // rotating row buffers of the contraction: [quad modulo (AHEAD + 1)][quantity][4 coefficients]
-  static constexpr int AHEAD = CATAPULT_PAIR_AHEAD;
+  static constexpr int AHEAD = 1;  // quads the shared-memory rows are loaded ahead of their use
   double rb[AHEAD + 1][4][4];
   static __device__ __forceinline__ constexpr int first_coef(int s, int q) {  // quad s = (a, b) descending
     return q * 64 + ((3 - s / 4) * 4 + (3 - s % 4)) * 4;
@@ -259,7 +264,7 @@ __device__ __forceinline__ void contraction_warp(const TraceConst& tc, unsigned 
     // ---- while the scalar warp is on its own: wait for the cell that is being fetched and load the rows the
     // first quads need (neither depends on the evaluation point), so that the request finds the thread ready
     pair_wait(pc);
-    if (__double2hiint(creg[DOI ? 63 : PT::NREG - 1]) == 0x7ffdead0) asm volatile("nanosleep.u32 1;");  // = wait for the loads
+    wait_for_register_loads(creg[DOI ? 63 : PT::NREG - 1]);
     if (!DOI) rows.preload(pc.strip_s);
     pbar_sync(bar0 + PB_REQ);
     const int rq = reqbuf[0];
@@ -873,8 +878,13 @@ catapult_status launch_trace_pair(const TraceConst& tc, const TraceArgs& a, int 
   }
 }
 
-catapult_status trace_pair_shape(int model, int64_t n, int* blocks, int* threads) {
+catapult_status trace_pair_shape(int model, bool doi, int64_t n, int* blocks, int* threads) {
   int cap = 0;
+  if (doi) {  // the derivative-of-interpolant kernels are other instantiations with their own register count
+    if (model == MODEL_BOOZER_VAC) return pair_shape<MODEL_BOOZER_VAC, MODE_ADAPTIVE, true>(n, blocks, threads, &cap);
+    if (model == MODEL_BOOZER_NV) return pair_shape<MODEL_BOOZER_NV, MODE_ADAPTIVE, true>(n, blocks, threads, &cap);
+    return pair_shape<MODEL_BOOZER_SAW, MODE_ADAPTIVE, true>(n, blocks, threads, &cap);
+  }
   if (model == MODEL_BOOZER_VAC) return pair_shape<MODEL_BOOZER_VAC, MODE_ADAPTIVE, false>(n, blocks, threads, &cap);
   if (model == MODEL_BOOZER_NV) return pair_shape<MODEL_BOOZER_NV, MODE_ADAPTIVE, false>(n, blocks, threads, &cap);
   return pair_shape<MODEL_BOOZER_SAW, MODE_ADAPTIVE, false>(n, blocks, threads, &cap);

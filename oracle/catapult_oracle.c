@@ -703,6 +703,57 @@ void orc_estimate(int g_kind, int64_t n, const int32_t *status, const double *ts
   out[2] = sum;
 }
 
+/* ---- other measurements g ("Similar functions g can be chosen to calculate energy loss ..., wall-loads
+ * from alpha particles"; readings G2, G3).  Both look at the END state of a trace only. ---- */
+
+/* Reading G2, lost energy: g_i = 1[lost] E_i / E_0 with the guiding-centre energy per unit mass at the exit point,
+ * E_i = vpar^2 / 2 + mu |B|(x_f) (mu = v_perp^2 / (2B) per unit mass), |B| from the tabulated field, and
+ * E_0 = v_total^2 / 2 the birth energy every particle shares.  Its mean (Eq. 2) is the fraction of the
+ * alpha power that leaves with lost particles; with a wave E_i differs from E_0. */
+void orc_lost_energy(const orc_field *f, const orc_params *p, int64_t n, const double *xf /*[4][n]*/,
+                     const double *mu /*[n]*/, const int32_t *status, double *g /*[n]*/) {
+  const double v = orc_vtotal(p);
+  const double E0 = 0.5 * v * v;
+  for (int64_t i = 0; i < n; ++i) {
+    if (status[i] != 1) { g[i] = 0.0; continue; }
+    const double x[4] = {xf[i], xf[n + i], xf[2 * n + i], xf[3 * n + i]};
+    double y[4];
+    orc_state_to_y(f, x, y);
+    const double B = orc_modB_at(f, y, NULL);
+    g[i] = (0.5 * x[3] * x[3] + mu[i] * B) / E0;
+  }
+}
+
+/* one histogram bin: u = (a - lo) / span, reduced to [0, 1) when periodic, bin = floor(u nb) clamped to [0, nb-1] */
+static int orc_bin(double a, double lo, double span, int periodic, int nb) {
+  double u = (a - lo) / span;
+  if (periodic) u = u - floor(u);
+  int b = (int)floor(u * (double)nb);
+  if (b < 0) b = 0;
+  if (b > nb - 1) b = nb - 1;
+  return b;
+}
+
+/* Reading G3, wall load: the number of lost particles per bin of the exit point, hist[nb0][nb1].
+ * Boozer: (theta over [0, 2 pi), zeta over one field period [lo2, hi2)), both periodic.
+ * Cylindrical: (phi = atan2(y, x) over one field period [lo2, hi2), periodic; Z over [lo1, hi1], clamped). */
+void orc_exit_histogram(const orc_field *f, int64_t n, const double *xf /*[4][n]*/, const int32_t *status,
+                        int nb0, int nb1, int64_t *hist /*[nb0][nb1]*/) {
+  for (int k = 0; k < nb0 * nb1; ++k) hist[k] = 0;
+  for (int64_t i = 0; i < n; ++i) {
+    if (status[i] != 1) continue;
+    int b0, b1;
+    if (f->coord == ORC_COORD_BOOZER) {
+      b0 = orc_bin(xf[n + i], f->lo[1], f->hi[1] - f->lo[1], 1, nb0);
+      b1 = orc_bin(xf[2 * n + i], f->lo[2], f->hi[2] - f->lo[2], 1, nb1);
+    } else {
+      b0 = orc_bin(atan2(xf[n + i], xf[i]), f->lo[2], f->hi[2] - f->lo[2], 1, nb0);
+      b1 = orc_bin(xf[2 * n + i], f->lo[1], f->hi[1] - f->lo[1], 0, nb1);
+    }
+    hist[b0 * nb1 + b1] += 1;
+  }
+}
+
 int orc_max_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -26,6 +26,9 @@
  *       retyped from the constants), explicit values win, dt0 clamped to dtmax.
  *   orc_trace                    : brute-force fixed-step RK4 on a tiny ensemble.
  *   orc_estimate                 : numpy.mean.
+ *   orc_lost_energy (G2)         : hand value from the closed-form |B| at a grid node; energy conservation in a
+ *       static field (g = 1 for every lost particle, interpolation-limited); 0 for particles that are not lost.
+ *   orc_exit_histogram (G3)      : numpy.histogram2d on independently reduced angles; hand-placed particles.
  * Parity unpinned: absolute loss fractions of the five configs (nothing in the
  * paper fixes them).
  */
@@ -86,6 +89,12 @@ typedef struct {
   int32_t loss_time_mode;      /* 0: end of the step that crossed (reading S5); 1: root inside it (reading S5b) */
   int32_t reserved_;
 } orc_params;
+
+/* ---- other measurements g (readings G2, G3) ---- */
+void orc_lost_energy(const orc_field *f, const orc_params *p, int64_t n, const double *xf, const double *mu,
+                     const int32_t *status, double *g);
+void orc_exit_histogram(const orc_field *f, int64_t n, const double *xf, const int32_t *status, int nb0, int nb1,
+                        int64_t *hist);
 
 /* ---- loss time inside the last step (reading S5b; tau, "the first time the particle
  * is observed beyond the boundary", sharpened) ---- */

@@ -335,5 +335,26 @@ def estimate(g_kind, status=None, tstop=None, g_user=None):
     return out
 
 
+def lost_energy(f: Field, p: CParams, xf, mu, status) -> np.ndarray:
+    """g_i = 1[lost] (vpar^2/2 + mu |B|(x_f)) / (v_total^2/2)  (reading G2)"""
+    xf, mu = _f64(xf), _f64(mu)
+    st = np.ascontiguousarray(status, dtype=np.int32)
+    n = st.size
+    g = np.zeros(n)
+    lib().orc_lost_energy(f.ref, C.byref(p), C.c_int64(n), _dp(xf), _dp(mu), st.ctypes.data_as(C.POINTER(C.c_int32)),
+                          _dp(g))
+    return g
+
+
+def exit_histogram(f: Field, xf, status, nb0: int, nb1: int) -> np.ndarray:
+    """lost particles per bin of the exit point (reading G3): int64 [nb0][nb1]"""
+    xf = _f64(xf)
+    st = np.ascontiguousarray(status, dtype=np.int32)
+    hist = np.zeros((nb0, nb1), dtype=np.int64)
+    lib().orc_exit_histogram(f.ref, C.c_int64(st.size), _dp(xf), st.ctypes.data_as(C.POINTER(C.c_int32)),
+                             C.c_int(nb0), C.c_int(nb1), hist.ctypes.data_as(C.POINTER(C.c_int64)))
+    return hist
+
+
 def max_threads() -> int:
     return int(lib().orc_max_threads())

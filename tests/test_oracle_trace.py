@@ -422,3 +422,105 @@ def test_cartesian_loss_is_the_first_accepted_state_beyond_the_closed_form_surfa
     # final states alone separates the two classes
     pf = _psi_closed_form(r["xf"])
     assert np.array_equal(pf >= edge, r["status"] == 1)
+
+
+def test_cartesian_loss_time_inside_the_step_ends_on_the_closed_form_surface(oracle):
+    """Reading S5b for the cylindrical model (sign change of the interpolated level function; the root
+    is looked for along the step's cubic Hermite interpolant, one table evaluation per bisection step).  Config 3's
+    level function is a quadratic, so the surface is known in closed form and the oracle's interpolation is not
+    needed to check it: with loss_time_mode 1 every lost particle ends ON the ellipse psi = psi_edge (from outside,
+    within the bisection's resolution), at a time inside the crossing step; statuses, step counts and the particles
+    that reach T are untouched; against a run at a 100x tighter tolerance the refined loss times of a loose run are
+    much closer than the unrefined ones."""
+    O = oracle
+    cfg = W.config(3, n=4, T=2e-5, ncell=[12, 11, 5])
+    f = O.Field(cfg["field"])
+    x0 = W.cyl_births(np.random.default_rng(13), 64, psi_frac=0.97)
+    edge = W.PSI_EDGE_CYL
+    loose0 = O.trace(f, O.make_params(dict(cfg["params"], rtol=1e-6)), x0)
+    loose1 = O.trace(f, O.make_params(dict(cfg["params"], rtol=1e-6, loss_time_mode=1)), x0)
+    tight1 = O.trace(f, O.make_params(dict(cfg["params"], rtol=1e-11, atol=1e-14, loss_time_mode=1)), x0)
+    assert np.array_equal(loose0["status"], loose1["status"]) and np.array_equal(loose0["nacc"], loose1["nacc"])
+    kept = loose0["status"] == 0
+    assert np.array_equal(loose0["xf"][:, kept], loose1["xf"][:, kept])
+    lost = np.flatnonzero((loose0["status"] == 1) & (tight1["status"] == 1))
+    assert len(lost) >= 10
+    psi0_, psi1_ = _psi_closed_form(loose0["xf"][:, lost]), _psi_closed_form(loose1["xf"][:, lost])
+    assert np.all(psi0_ >= edge) and np.median(psi0_ / edge - 1) > 1e-6      # mode 0 ends well beyond the surface
+    assert np.all(psi1_ >= edge * (1 - 1e-13)) and np.all(psi1_ < edge * (1 + 1e-9))   # mode 1 ends on it
+    assert np.all(loose1["tstop"][lost] <= loose0["tstop"][lost]) and np.all(loose1["tstop"][lost] > 0)
+    e0 = np.abs(loose0["tstop"][lost] - tight1["tstop"][lost])
+    e1 = np.abs(loose1["tstop"][lost] - tight1["tstop"][lost])
+    assert np.median(e1) < 0.05 * np.median(e0), (np.median(e1), np.median(e0))
+    # the crossing step brackets the refined time (trajectory record of mode 0: its last two rows are the step's ends)
+    for i in lost[:16]:
+        traj, ts, st = O.trace_record(f, O.make_params(dict(cfg["params"], rtol=1e-6)), x0[:, i])
+        assert traj[-2, 0] < loose1["tstop"][i] <= traj[-1, 0]
+
+
+def test_lost_energy_measurement(oracle):
+    """Reading G2 ("energy loss"): g = 1[lost] (vpar^2/2 + mu |B|(x_f)) / (v_total^2/2).
+    (1) Hand value: a "lost" particle placed ON a grid node, where the interpolant returns the nodal value, which
+    is the closed-form |B| of the workload (workloads.boozer_field_values) -- the oracle's interpolation does not
+    enter the expected number.  (2) A particle that is not lost contributes 0 whatever its state.  (3) In a static
+    field the guiding-centre energy is an invariant: every particle the tracer loses left with the energy it was
+    born with, g = 1 to the interpolation-limited drift (a few 1e-6 on config 0's grid, reading Q3).  A dropped
+    mu |B| term, a missing factor 1/2 or |B| taken at the wrong point fails (1) or (3)."""
+    O = oracle
+    cfg = W.config(0, n=64, T=1e-4)
+    f, p = O.Field(cfg["field"]), O.make_params(cfg["params"])
+    k = cfg["field"]["ncell"]
+    node = (37, 20, 11)                                           # unique-node indices (s, theta, zeta)
+    s, th, ze = node[0] / (3.0 * k[0]), 2 * math.pi * node[1] / (3.0 * k[1]), (2 * math.pi / W.NFP) * node[2] / (3.0 * k[2])
+    B = float(W.boozer_field_values(cfg["field"]["modes"], s, th, ze)[0])
+    assert B == cfg["field"]["nodes"][0][node]
+    vpar, mu = 0.3 * W.V_TOTAL, 0.41 * W.V_TOTAL ** 2 / B
+    xf = np.array([[s, 0.5], [th, 1.0], [ze, 0.2], [vpar, vpar]])
+    g = O.lost_energy(f, p, xf, np.array([mu, mu]), np.array([1, 0], dtype=np.int32))
+    assert abs(g[0] - (0.5 * 0.09 + 0.41) / 0.5) < 1e-13 and g[1] == 0.0
+    r = O.trace(f, p, cfg["x0"])
+    mu0 = np.array([O.mu_init(f, p, cfg["x0"][:, i]) for i in range(64)])
+    g = O.lost_energy(f, p, r["xf"], mu0, r["status"])
+    lost = r["status"] == 1
+    assert lost.sum() >= 1 and np.all(g[~lost] == 0.0)
+    assert np.all(np.abs(g[lost] - 1.0) < 2e-5)
+    est = O.estimate(2, g_user=g)
+    assert abs(est[0] - lost.mean()) < 2e-5 * max(lost.mean(), 1e-3)      # lost power fraction ~ loss fraction here
+
+
+def test_exit_histogram_matches_numpy(oracle):
+    """Reading G3 ("wall-loads"): lost particles per bin of the exit point.  Against numpy.histogram2d on
+    angles reduced with np.mod (a library routine and an independent reduction), on both coordinate systems; hand-placed
+    particles land in the bins worked out by hand; particles that are not lost are not counted; values outside a
+    non-periodic range fall into the end bins."""
+    O = oracle
+    rng = np.random.default_rng(21)
+    n = 5000
+    status = (rng.random(n) < 0.6).astype(np.int32)
+    # Boozer: theta in (-pi, pi], zeta unreduced (as catapult_trace returns them)
+    cfg = W.config(0, n=1, T=1e-6)
+    f = O.Field(cfg["field"])
+    xf = np.array([1.0 + 0.01 * rng.random(n), rng.uniform(-math.pi, math.pi, n), rng.uniform(-40.0, 40.0, n), rng.normal(size=n)])
+    per = 2 * math.pi / W.NFP
+    h = O.exit_histogram(f, xf, status, 12, 7)
+    lost = status == 1
+    want, _, _ = np.histogram2d(np.mod(xf[1][lost], 2 * math.pi), np.mod(xf[2][lost], per), bins=[12, 7],
+                                range=[[0, 2 * math.pi], [0, per]])
+    assert h.sum() == lost.sum() and np.array_equal(h, want.astype(np.int64))
+    hand = np.array([[1.0, 1.0, 1.0], [0.1, -0.1, math.pi - 1e-9], [0.5 * per / 7, per + 2.5 * per / 7, -0.5 * per / 7], [0, 0, 0]])
+    hh = O.exit_histogram(f, hand, np.array([1, 1, 1], dtype=np.int32), 12, 7)
+    assert hh[0, 0] == 1 and hh[11, 2] == 1 and hh[5, 6] == 1 and hh.sum() == 3
+    # cylindrical: phi from (x, y), Z clamped into the grid's range
+    c3 = W.config(3, n=1, T=1e-6, ncell=[4, 4, 2])
+    f3 = O.Field(c3["field"])
+    R, phi = rng.uniform(6.0, 9.5, n), rng.uniform(-math.pi, math.pi, n)
+    zlo, zhi = c3["field"]["lo"][1], c3["field"]["hi"][1]
+    Z = rng.uniform(1.2 * zlo, 1.2 * zhi, n)
+    x3 = np.array([R * np.cos(phi), R * np.sin(phi), Z, rng.normal(size=n)])
+    h3 = O.exit_histogram(f3, x3, status, 16, 9)
+    want3, _, _ = np.histogram2d(np.mod(phi[lost], 2 * math.pi), np.clip(Z[lost], zlo, np.nextafter(zhi, zlo)), bins=[16, 9],
+                                 range=[[0, 2 * math.pi], [zlo, zhi]])
+    assert h3.sum() == lost.sum()
+    # numpy's bin edges are lo + k (hi - lo) / nb, the oracle's rule is floor((a - lo) / span * nb): equal except for
+    # a point within a rounding of an edge; none of the 3000 seeded points is
+    assert np.array_equal(h3, want3.astype(np.int64))

@@ -206,13 +206,14 @@ def committed_capture(model: str) -> dict:
     (profiles/r2_traffic_pair.csv; the command is in the .md beside it).  bench.py does not run ncu: the traffic
     it reports is that capture's per-evaluation figure times the evaluations of its own timed launches."""
     out = {}
-    try:
-        for line in open(os.path.join(ROOT, "profiles", "r2_traffic_pair.csv")):
-            f = line.strip().split(",")
-            if len(f) >= 3 and f[0] == model:
-                out[f[1]] = float(f[2])
-    except Exception:
-        pass
+    for name in ("r2_traffic_pair.csv", "r3_traffic.csv"):   # boozer_saw (round 2); cart, boozer_vac (round 3)
+        try:
+            for line in open(os.path.join(ROOT, "profiles", name)):
+                f = line.strip().split(",")
+                if len(f) >= 3 and f[0] == model:
+                    out[f[1]] = float(f[2])
+        except Exception:
+            pass
     return out
 
 
@@ -391,7 +392,7 @@ def main():
                                      "note": "exactly known flops of the tricubic contraction alone; locate, right-hand "
                                              "side and stage algebra excluded"},
                 "traffic": dram_b * evals_per_launch if dram_b else None,
-                "traffic_source": "profiles/r2_traffic_pair.csv (committed ncu --set full capture, bytes per evaluation) "
+                "traffic_source": "profiles/r2_traffic_pair.csv / r3_traffic.csv (committed ncu --set full captures, bytes per evaluation) "
                                   "x the evaluations of one timed launch" if dram_b else None,
                 "rhs_evals_per_launch": evals_per_launch,
                 "launch_ms": sum(trace_ms) / max(1, len(trace_ms)),

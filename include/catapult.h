@@ -122,8 +122,10 @@ typedef struct {
   int32_t loss_time_mode;      /* loss time tau: 0 = end time of the first accepted step that ends
                                   beyond the boundary, the end state returned (S5); 1 = root inside that
                                   step: cubic Hermite interpolant of the stepped variables through the step's end
-                                  states and end derivatives, bisected to the first observed point with s >= 1,
-                                  that point and its time returned (S5b; Boozer only)        */
+                                  states and end derivatives, bisected to the first observed point beyond the
+                                  boundary (Boozer: s >= 1; cylindrical: interpolated level function >= psi_edge,
+                                  one table evaluation per bisection step), that point and its time
+                                  returned (S5b)                                              */
   int32_t reserved_;           /* 0                                                              */
 } catapult_trace_params;
 
@@ -235,6 +237,27 @@ catapult_status catapult_step_once(const catapult_field *f, const catapult_trace
 catapult_status catapult_estimate(int32_t g_kind, int64_t n, const int32_t *d_status,
                                   const double *d_tstop, const double *d_g_user, double *d_out,
                                   double *h_out, void *stream);
+
+/* ---- other measurements g on the end states ("Similar functions g can be chosen to calculate energy
+ * loss ..., wall-loads from alpha particles"; readings G2, G3) ---------------------------------------
+ * catapult_measure_lost_energy: d_g[i] = 1[status LOST] * (vpar^2/2 + mu_i |B|(x_f,i)) / (v_total^2/2): the energy a
+ * lost particle leaves with, in units of the birth energy all particles share, |B| from the field's
+ * tables at the exit point d_xf[4][n] (as returned by the tracing calls), d_mu[n] the magnetic moment per unit mass
+ * (catapult_trace_init / catapult_trace_continue keep it).  Feed d_g to catapult_estimate with g_kind 2: the mean is
+ * the fraction of the alpha power lost (equal to the loss fraction in a static field, not with a wave).
+ * Errors: EINVAL (NULL, n < 0, bad params as in catapult_trace, another device), ECUDA. */
+catapult_status catapult_measure_lost_energy(const catapult_field *f, const catapult_trace_params *p, int64_t n,
+                                             const double *d_xf, const double *d_mu, const int32_t *d_status,
+                                             double *d_g, void *stream);
+/* catapult_exit_histogram: the wall-load stand-in.  d_hist[nbins0][nbins1] (uint64, zeroed by the call) = number of
+ * LOST particles per bin of the exit point: Boozer (theta over [0, 2pi), zeta over one field period), both periodic;
+ * cylindrical (phi = atan2(y, x) over one field period, periodic; Z over the grid's [lo, hi], end bins collect what
+ * lies outside).  Bin of a coordinate a: u = (a - lo) / (hi - lo), minus floor(u) when periodic, floor(u * nbins)
+ * clamped to [0, nbins-1], each operation rounded once.  Exact integer counts whatever the launch order.
+ * Errors: EINVAL (NULL, n < 0, nbins < 1 or more than 2^24 bins, another device), ECUDA. */
+catapult_status catapult_exit_histogram(const catapult_field *f, int64_t n, const double *d_xf,
+                                        const int32_t *d_status, int32_t nbins0, int32_t nbins1, uint64_t *d_hist,
+                                        void *stream);
 
 /* ---- the estimate for callers that must not allocate device memory ------------------------------
  * catapult_estimate above takes a few KiB of device scratch from the stream-ordered allocator on every call.

@@ -28,7 +28,8 @@ EXPORTS = [
     "catapult_field_table_bytes", "catapult_field_eval", "catapult_field_export_rows",
     "catapult_trace", "catapult_trace_init", "catapult_trace_continue", "catapult_trace_host",
     "catapult_trace_continue_host", "catapult_release_host_cache", "catapult_trace_scripted",
-    "catapult_step_once", "catapult_estimate", "catapult_estimate_static", "catapult_trace_launch_shape", "catapult_last_error",
+    "catapult_step_once", "catapult_estimate", "catapult_estimate_static", "catapult_measure_lost_energy",
+    "catapult_exit_histogram", "catapult_trace_launch_shape", "catapult_last_error",
     "catapult_version",
 ]
 PROBE_EXPORTS = ["catapult_math_probe", "catapult_measure_fp64_peak", "catapult_measure_l2_bandwidth",
@@ -89,6 +90,8 @@ def load():
     L.catapult_step_once.argtypes = [vp, C.POINTER(TraceParams), i64, dp, dp, dp, dp, dp, dp, vp]
     L.catapult_estimate.argtypes = [C.c_int32, i64, dp, dp, dp, dp, dp, vp]
     L.catapult_estimate_static.argtypes = [C.c_int32, i64, dp, dp, dp, dp, vp]
+    L.catapult_measure_lost_energy.argtypes = [vp, C.POINTER(TraceParams), i64, dp, dp, dp, dp, vp]
+    L.catapult_exit_histogram.argtypes = [vp, i64, dp, dp, C.c_int32, C.c_int32, dp, vp]
     L.catapult_release_host_cache.argtypes = []
     L.catapult_trace_launch_shape.argtypes = [vp, C.POINTER(TraceParams), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     L.catapult_last_error.restype = C.c_char_p
@@ -379,6 +382,28 @@ def catapult_estimate(g_kind: int, d_status=None, d_tstop=None, d_g_user=None, t
     _check(load().catapult_estimate(g_kind, n, _ptr(d_status, torch.int32, True), _ptr(d_tstop, torch.float64, True),
                                     _ptr(d_g_user, torch.float64, True), _ptr(out), _hptr(h, np.float64), _stream()))
     return h if to_host else out
+
+
+def catapult_measure_lost_energy(f: Field, pd: dict, d_xf, d_mu, d_status):
+    """g[i] = 1[lost] (vpar^2/2 + mu |B|(x_f)) / (v_total^2/2) as a CUDA float64[n] tensor (feed it to
+    catapult_estimate(2, d_g_user=g))."""
+    torch = _torch()
+    p = make_params(pd)
+    n = d_xf.shape[1]
+    g = torch.empty(n, dtype=torch.float64, device=d_xf.device)
+    _check(load().catapult_measure_lost_energy(f._h, C.byref(p), n, _ptr(d_xf, torch.float64), _ptr(d_mu, torch.float64),
+                                               _ptr(d_status, torch.int32), _ptr(g), _stream()))
+    return g
+
+
+def catapult_exit_histogram(f: Field, d_xf, d_status, nbins0: int, nbins1: int):
+    """Lost particles per bin of the exit point: CUDA int64[nbins0][nbins1]."""
+    torch = _torch()
+    n = d_xf.shape[1]
+    hist = torch.empty((nbins0, nbins1), dtype=torch.int64, device=d_xf.device)
+    _check(load().catapult_exit_histogram(f._h, n, _ptr(d_xf, torch.float64), _ptr(d_status, torch.int32), nbins0, nbins1,
+                                          _ptr(hist), _stream()))
+    return hist
 
 
 ESTIMATE_STATIC_MAX_N = 2097152

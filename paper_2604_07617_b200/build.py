@@ -18,7 +18,7 @@ INC = os.path.join(ROOT, "include")
 LIB = os.path.join(PKG, "libcatapult.so")
 PROBE_LIB = os.path.join(PKG, "libcatapult_probe.so")
 OBJ = os.path.join(PKG, "build")
-SOURCES = ["api.cu", "field.cu", "tracer.cu", "tracer_pair.cu", "estimate.cu"]
+SOURCES = ["api.cu", "field.cu", "tracer.cu", "tracer_pair.cu", "estimate.cu", "measure.cu"]
 PROBE_SOURCES = ["probe_api.cu", "peaks.cu", "mathprobe.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]

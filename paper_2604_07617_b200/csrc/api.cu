@@ -114,8 +114,6 @@ static catapult_status make_trace_const(const catapult_field* f, const catapult_
   if (p->max_steps < 0 || p->max_consecutive_rejects < 0)
     return fail(CATAPULT_EINVAL, "max_steps / max_consecutive_rejects must be >= 0");
   if (p->loss_time_mode != 0 && p->loss_time_mode != 1) return fail(CATAPULT_EINVAL, "loss_time_mode must be 0 or 1");
-  if (p->loss_time_mode == 1 && f->desc.coord != CATAPULT_COORD_BOOZER)
-    return fail(CATAPULT_EUNSUPPORTED, "loss_time_mode 1 (loss time inside the step) is built for Boozer tracing only");
   if (p->saw_on) {
     if (f->desc.coord != CATAPULT_COORD_BOOZER)
       return fail(CATAPULT_EUNSUPPORTED, "the shear Alfven wave is built for Boozer tracing only");
@@ -598,6 +596,33 @@ catapult_status catapult_estimate(int32_t g_kind, int64_t n, const int32_t* d_st
     CATAPULT_CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
   }
   return CATAPULT_OK;
+}
+
+catapult_status catapult_measure_lost_energy(const catapult_field* f, const catapult_trace_params* p, int64_t n,
+                                             const double* d_xf, const double* d_mu, const int32_t* d_status,
+                                             double* d_g, void* stream) {
+  if (n < 0) return fail(CATAPULT_EINVAL, "n < 0");
+  if (n > 0 && (!d_xf || !d_mu || !d_status || !d_g)) return fail(CATAPULT_EINVAL, "d_xf, d_mu, d_status and d_g are required");
+  TraceConst tc;
+  int model = 0;
+  catapult_status st = make_trace_const(f, p, &tc, &model);  // validates field and parameters; v_total^2
+  if (st != CATAPULT_OK) return st;
+  st = use_field_on(f, (cudaStream_t)stream);
+  if (st != CATAPULT_OK) return st;
+  return launch_lost_energy(f->fc, 2.0 / tc.vtot2, n, d_xf, d_mu, d_status, d_g, (cudaStream_t)stream);
+}
+
+catapult_status catapult_exit_histogram(const catapult_field* f, int64_t n, const double* d_xf, const int32_t* d_status,
+                                        int32_t nbins0, int32_t nbins1, uint64_t* d_hist, void* stream) {
+  if (!f) return fail(CATAPULT_EINVAL, "field is NULL");
+  if (n < 0) return fail(CATAPULT_EINVAL, "n < 0");
+  if (nbins0 < 1 || nbins1 < 1 || (int64_t)nbins0 * nbins1 > (int64_t)1 << 24)
+    return fail(CATAPULT_EINVAL, "nbins0, nbins1 must be >= 1 with at most 2^24 bins in all");
+  if (!d_hist || (n > 0 && (!d_xf || !d_status))) return fail(CATAPULT_EINVAL, "d_xf, d_status and d_hist are required");
+  catapult_status st = use_device_of(f);  // geometry only: the tables are not read
+  if (st != CATAPULT_OK) return st;
+  return launch_exit_histogram(f->fc, n, d_xf, d_status, nbins0, nbins1, reinterpret_cast<unsigned long long*>(d_hist),
+                               (cudaStream_t)stream);
 }
 
 // The estimate without any allocation (include/catapult.h): same validation as catapult_estimate, the size limit and

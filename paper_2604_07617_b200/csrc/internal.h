@@ -85,6 +85,12 @@ catapult_status launch_estimate(int g_kind, int64_t n, const int* d_status, cons
 catapult_status launch_estimate_static(int g_kind, int64_t n, const int* d_status, const double* d_tstop,
                                        const double* d_g, double* d_out, cudaStream_t s);
 
+// measure.cu
+catapult_status launch_lost_energy(const FieldConst& fc, double inv_E0, int64_t n, const double* d_xf, const double* d_mu,
+                                   const int* d_status, double* d_g, cudaStream_t s);
+catapult_status launch_exit_histogram(const FieldConst& fc, int64_t n, const double* d_xf, const int* d_status, int nb0,
+                                      int nb1, unsigned long long* d_hist, cudaStream_t s);
+
 // mathprobe.cu
 catapult_status launch_math_probe(int fn, int64_t n, const double* d_a, const double* d_b, double* d_o0, double* d_o1,
                                   cudaStream_t s);

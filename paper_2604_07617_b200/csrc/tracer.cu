@@ -239,6 +239,38 @@ struct ScalarRegs {   // what the scalar warp carries from round to round beside
   unsigned n_block;   // ... of which after the point had been located (the guess missed)
 };
 
+// Loss time inside the crossing step for the cylindrical model (include/catapult.h loss_time_mode 1, S5b;
+// the loss test is a sign change of the INTERPOLATED level function, column 6).  Same construction as
+// loss_refine_boozer (gc_device.cuh): the cubic Hermite interpolant through the step's end states and end derivatives,
+// 48 bisections from [0, 1] on "level(y(theta)) >= psi_edge", the smallest theta observed beyond the boundary returned
+// and y(theta) left in yb.  The level at an interior point needs a table evaluation; the lost lane does it by itself
+// straight from the table (locate + the 63-FMA Horner form every user of the table follows, as catapult_field_eval),
+// not through the contraction warps: it runs once per lost particle, out of line, so that the stepping loop keeps its
+// registers.
+__device__ __noinline__ double loss_refine_cart(const FieldConst& f, const double ya[4], const double ka[4],
+                                                double yb[4], const double kb[4], double h) {
+  using AX = AxisRoles<false>;
+  double lo = 0.0, hi = 1.0, ym[4];
+#pragma unroll 1
+  for (int it = 0; it < 48; ++it) {
+    const double mid = 0.5 * (lo + hi);
+    hermite_state(ya, ka, yb, kb, h, mid, ym);
+    double R, invR, w[3];
+    fm::sqrt_rsqrt(fma(ym[0], ym[0], ym[1] * ym[1]), R, invR);
+    const int cell = locate<false>(f, R, ym[2], fm::atan2(ym[1], ym[0]), w);
+    const double* src = f.table + ((long long)cell * CATAPULT_NQUANT_CYL + (CATAPULT_NQUANT_CYL - 1)) * 64;
+    const double level = horner64(
+        [&](int e, double& f0, double& f1, double& f2, double& f3) { ldg_f64x4(src + e, f0, f1, f2, f3); },
+        w[AX::LAST], w[AX::SECOND], w[AX::FIRST]);
+    if (level >= f.psi0) hi = mid;
+    else lo = mid;
+  }
+  hermite_state(ya, ka, yb, kb, h, hi, ym);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) yb[i] = ym[i];
+  return hi;
+}
+
 // One lock-step right-hand-side evaluation of the scalar warp at the point (tr, X): see the top of this file.
 // Lanes with act = false publish a request nobody serves.  ratio >= 0: the next point is expected at
 // X + ratio (X - start of the attempt) and its cell is fetched ahead.  All 32 lanes must call this.
@@ -583,7 +615,21 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
           } else {
             consecutive = 0;
             ++nacc;
-            t = clamped ? tc.T : t + h;
+            const bool lost = is_lost<MODEL>(tc, level);
+            if (lost && tc.loss_time_mode == 1) {
+              // DESIGN.md S5b: the loss time and state inside this step
+              const double ya[4] = {ysm[0], ysm[32], ysm[64], ysm[96]};
+              const double ka[4] = {ks[0], ks[32], ks[64], ks[96]};
+              // copies: only arrays of this rare branch have their address taken, X and dy stay in registers
+              double yb[4] = {X[0], X[1], X[2], X[3]};
+              const double kb[4] = {dy[0], dy[1], dy[2], dy[3]};
+              const double theta = loss_refine_cart(tc.f, ya, ka, yb, kb, h);  // yb <- y(theta)
+#pragma unroll
+              for (int c = 0; c < 4; ++c) X[c] = yb[c];
+              t = __dadd_rn(t, __dmul_rn(theta, h));
+            } else {
+              t = clamped ? tc.T : t + h;
+            }
             if (!clamped) dt = dtn;
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
@@ -591,7 +637,7 @@ trace_kernel(const __grid_constant__ TraceConst tc, const __grid_constant__ Trac
               ks[c * 32] = dy[c];  // first-same-as-last
             }
             // DESIGN.md S5: loss first, then T
-            if (is_lost<MODEL>(tc, level)) finish = CATAPULT_ST_LOST;
+            if (lost) finish = CATAPULT_ST_LOST;
             else if (MODE != MODE_SCRIPT && t >= tc.T) finish = CATAPULT_ST_REACHED_T;
           }
         }

@@ -833,9 +833,7 @@ def test_loss_time_inside_the_step(K, oracle, cases, idx):
 
 
 def test_loss_time_mode_is_validated(K, cases):
-    c3, c0 = cases[3], cases[0]
-    with pytest.raises(K.CatapultError):   # cylindrical model: not built
-        K.catapult_trace(c3["gf"], dict(c3["cfg"]["params"], loss_time_mode=1), _dev(c3["cfg"]["x0"]))
+    c0 = cases[0]
     with pytest.raises(K.CatapultError):
         K.catapult_trace(c0["gf"], dict(c0["cfg"]["params"], loss_time_mode=2), _dev(c0["cfg"]["x0"]))
 
@@ -1229,3 +1227,119 @@ def test_loss_time_inside_the_step_on_the_other_boozer_variants(K, oracle, nonva
           f"of the step, state {worst:.2e}")
     assert nlost >= 6
     assert worst_t <= bar and worst <= bar
+
+
+@pytest.mark.parametrize("rtol", [1e-9, 1e-6])
+def test_cartesian_loss_time_inside_the_step(K, oracle, cases, rtol):
+    """loss_time_mode 1 for the cylindrical model (SURVEY 8(f) f3 "sharper tau"): the root of the
+    INTERPOLATED level function along the crossing step's Hermite interpolant, one table evaluation per bisection step
+    (tracer.cu loss_refine_cart; oracle orc_loss_refine, pinned by the closed-form surface in
+    tests/test_oracle_trace.py).  Scripted replay of the oracle's step sequence: statuses exact; the loss time (as a
+    fraction of the crossing step, times the relative change of the level across the step -- the root moves by the
+    difference of the interpolated levels divided by d level / d theta) and the state to 1e-8; every lost particle
+    ends on the closed-form surface.  Adaptive run: the mode touches nothing but the stop time and state of lost
+    particles."""
+    c = cases[3]
+    cfg = c["cfg"]
+    x0 = np.concatenate([W.cyl_births(np.random.default_rng(13), 40, psi_frac=0.97), cfg["x0"][:, :10]], axis=1)
+    n = x0.shape[1]
+    p0 = dict(cfg["params"], T=2e-5, rtol=rtol)
+    p1 = dict(p0, loss_time_mode=1)
+    op0, op1 = oracle.make_params(p0), oracle.make_params(p1)
+    recs = [oracle.trace_record(c["of"], op0, x0[:, i]) for i in range(n)]
+    hs = [np.diff(r[0][:, 0]) for r in recs]
+    H = np.zeros((max(len(h) for h in hs) + 1, n))
+    for i, h in enumerate(hs):
+        H[:len(h), i] = h
+    g = K.catapult_trace_scripted(c["gf"], p1, _dev(x0), _dev(H))
+    gx, gt, gs = (g[k].cpu().numpy() for k in ("xf", "tstop", "status"))
+    edge = W.PSI_EDGE_CYL
+    psi = lambda x: (W.B0 / (2.0 * W.Q0_CYL)) * ((np.hypot(x[0], x[1]) - W.R0) ** 2 + (x[2] / W.KAPPA_CYL) ** 2)  # noqa: E731
+    sc = _state_scale(1)
+    nlost, worst, worst_t = 0, 0.0, 0.0
+    for i in range(n):
+        xo, to, so, _ = oracle.trace_scripted(c["of"], op1, x0[:, i], hs[i])
+        assert gs[i] == so
+        if so != 1:
+            assert gt[i] == to
+            continue
+        nlost += 1
+        hlast = hs[i][-1]
+        assert recs[i][1] - hlast < to <= recs[i][1]                    # inside the crossing step
+        dlevel = abs(psi(recs[i][0][-1, 1:5]) - psi(recs[i][0][-2, 1:5])) / edge
+        worst_t = max(worst_t, abs(gt[i] - to) / hlast * dlevel)
+        worst = max(worst, (np.abs(gx[:, i] - xo) / np.maximum(sc, np.abs(xo))).max())
+        assert edge * (1 - 1e-13) <= psi(gx[:, i]) < edge * (1 + 1e-9)
+    print(f"cfg3 rtol {rtol:g}: {nlost} lost; loss time inside the step: worst difference x level change {worst_t:.2e} "
+          f"of the step, state {worst:.2e}")
+    assert nlost >= 10
+    assert worst_t <= 1e-8 and worst <= 1e-8
+    g0 = K.catapult_trace(c["gf"], p0, _dev(x0))
+    g1 = K.catapult_trace(c["gf"], p1, _dev(x0))
+    s0, s1 = g0["status"].cpu().numpy(), g1["status"].cpu().numpy()
+    assert np.array_equal(s0, s1) and np.array_equal(g0["nacc"].cpu().numpy(), g1["nacc"].cpu().numpy())
+    kept, lost = s0 == 0, s0 == 1
+    assert np.array_equal(g0["xf"].cpu().numpy()[:, kept], g1["xf"].cpu().numpy()[:, kept])
+    t0, t1 = g0["tstop"].cpu().numpy(), g1["tstop"].cpu().numpy()
+    assert np.all(t1[lost] <= t0[lost]) and np.any(t1[lost] < t0[lost])
+    pe = psi(g1["xf"].cpu().numpy()[:, lost])
+    assert np.all((pe >= edge * (1 - 1e-13)) & (pe < edge * (1 + 1e-9)))
+    o1 = oracle.trace(c["of"], op1, x0)
+    assert np.array_equal(s1, o1["status"]) and np.allclose(t1[lost], o1["tstop"][lost], rtol=1e-4, atol=0.0)
+
+
+# ---- f3: other measurements g on the end states (PAPER.md:25; DESIGN.md G2, G3) --------------------------------------
+@pytest.mark.parametrize("idx", [2, 3, 4])
+def test_lost_energy_and_exit_histogram_parity(K, oracle, cases, idx):
+    """catapult_measure_lost_energy / catapult_exit_histogram on the device's own trace against orc_lost_energy /
+    orc_exit_histogram on the same end states: g to 1e-12 (one table evaluation), the histogram's integer counts
+    bit-exact (the bin is decided by the same singly rounded operations on both sides; for the cylindrical model phi
+    comes from atan2, where the two libraries may differ in the last place: the test also checks that no exit point
+    lies within 1e-9 of a bin edge, so that the counts are unique).  The magnetic moment the device keeps is the
+    oracle's orc_mu_init to 1e-13.  With the estimate (g_kind 2) on top: the lost power fraction, which in a static
+    field equals the loss fraction up to the interpolation error of |B| and with the wave (config 4) does not have to."""
+    c = cases[idx]
+    cfg = c["cfg"]
+    coord = cfg["field"]["coord"]
+    x0 = np.tile(cfg["x0"], (1, 8))[:, :257]
+    if coord == 0:
+        x0[0, ::2] = 0.985 + 0.014 * np.linspace(0.0, 1.0, len(x0[0, ::2]))
+    else:
+        x0[:, ::2] = W.cyl_births(np.random.default_rng(44), x0[:, ::2].shape[1], psi_frac=0.97)
+    pd = dict(cfg["params"], T=2e-5)
+    st = K.catapult_trace_init(c["gf"], pd, _dev(x0).clone())
+    mu_o = np.array([oracle.mu_init(c["of"], c["op"], x0[:, i]) for i in range(x0.shape[1])])
+    assert np.allclose(st["mu"].cpu().numpy(), mu_o, rtol=1e-13, atol=0.0)
+    K.catapult_trace_continue(c["gf"], pd, st)
+    xf, status = st["x"].cpu().numpy(), st["status"].cpu().numpy()
+    lost = status == 1
+    assert 20 <= lost.sum() <= 200
+    g = K.catapult_measure_lost_energy(c["gf"], pd, st["x"], st["mu"], st["status"])
+    go = oracle.lost_energy(c["of"], c["op"], xf, st["mu"].cpu().numpy(), status)
+    gg = g.cpu().numpy()
+    assert np.all(gg[~lost] == 0.0) and np.allclose(gg, go, rtol=1e-12, atol=0.0)
+    est = K.catapult_estimate(2, d_g_user=g)
+    eo = oracle.estimate(2, g_user=go)
+    assert np.allclose(est[:3], eo, rtol=1e-12)
+    if idx != 4:
+        # static field: the energy is invariant up to the interpolation error of |B|, which on these deliberately
+        # coarse, ragged test grids (modes up to m = 8 on 12 x 10 x 9 cells, exit points extrapolated beyond s = 1) is
+        # a few per cent; the tight form of this check (2e-5 on config 0's own grid) is the oracle's pin
+        assert np.all(np.abs(gg[lost] - 1.0) < (0.1 if coord == 0 else 1e-6))
+    nb0, nb1 = 24, 10
+    h = K.catapult_exit_histogram(c["gf"], st["x"], st["status"], nb0, nb1).cpu().numpy()
+    ho = oracle.exit_histogram(c["of"], xf, status, nb0, nb1)
+    lo, hi = cfg["field"]["lo"], cfg["field"]["hi"]
+    if coord == 0:
+        u = np.mod((xf[1][lost] - lo[1]) / (hi[1] - lo[1]), 1.0) * nb0
+    else:
+        u = np.mod((np.arctan2(xf[1][lost], xf[0][lost]) - lo[2]) / (hi[2] - lo[2]), 1.0) * nb0
+    assert np.min(np.abs(u - np.round(u))) > 1e-9
+    assert h.sum() == lost.sum() and np.array_equal(h, ho)
+    print(f"cfg{idx}: {int(lost.sum())} lost; lost power fraction {est[0]:.5f} (loss fraction {lost.mean():.5f}); "
+          f"histogram {np.count_nonzero(h)} of {nb0 * nb1} bins hit")
+    # empty ensemble, bad arguments
+    e = torch.empty((4, 0), dtype=torch.float64, device="cuda")
+    assert K.catapult_exit_histogram(c["gf"], e, torch.empty(0, dtype=torch.int32, device="cuda"), 3, 2).sum().item() == 0
+    with pytest.raises(K.CatapultError):
+        K.catapult_exit_histogram(c["gf"], st["x"], st["status"], 0, 4)

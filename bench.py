@@ -500,7 +500,7 @@ def main():
             "config": {"workload": cfg["name"], "particles_per_gpu": npart, "window_s": args.window,
                        "T_full_s": W.FULL_T[cfg_idx], "ncell": fd["ncell"], "model": model,
                        "rtol": pd["rtol"], "atol": pd["atol"], "table_bytes": table_bytes,
-                       "l2_policy": "inputs larger than L2 (512 MiB tables, 126 MB L2)" if table_bytes > (126 << 20)
+                       "l2_policy": f"inputs larger than L2 ({table_bytes >> 20} MiB tables, 126 MB L2)" if table_bytes > (126 << 20)
                        else "tables fit in L2 (resident by design)",
                        "launch": {"blocks": blocks, "threads": threads},
                        "parallelism": f"dp{world} (one ensemble of {npart * world} particles split by interleaved "
